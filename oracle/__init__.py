@@ -1,0 +1,176 @@
+"""FP64 CPU oracle for cRMSD -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` / `--impl reference`
+legs may import this package.  It shares no code with `paper_1302_4000_b200/` (the CUDA path)
+and imports nothing from it.
+
+`oracle.crmsd_oracle.c` is the oracle proper (plain C, double precision, Jacobi SVD per pair; see
+its header for the algorithm and the PAPER.md citations).  This file only builds it with gcc and
+marshals numpy arrays through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "crmsd_oracle.c")
+_LIB = os.path.join(_HERE, "libcrmsd_oracle.so")
+_lib = None
+
+_f32p = ctypes.POINTER(ctypes.c_float)
+_f64p = ctypes.POINTER(ctypes.c_double)
+_i64p = ctypes.POINTER(ctypes.c_int64)
+
+
+def build(force: bool = False) -> str:
+    """Compile crmsd_oracle.c -> libcrmsd_oracle.so (gcc -O2 -fopenmp, no fast-math)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.run(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"],
+                       check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.oracle_center.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, _f64p, _f64p]
+        lib.oracle_center.restype = None
+        for name in ("oracle_crmsd_pair",):
+            f = getattr(lib, name)
+            f.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p]
+            f.restype = ctypes.c_double
+        lib.oracle_crmsd_pair_eq2.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p, _f64p, _f64p]
+        lib.oracle_crmsd_pair_eq2.restype = ctypes.c_double
+        lib.oracle_crmsd_pair_eq1.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p, _f64p]
+        lib.oracle_crmsd_pair_eq1.restype = ctypes.c_double
+        lib.oracle_pair_spectrum.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p, _f64p, _f64p]
+        lib.oracle_pair_spectrum.restype = None
+        lib.oracle_crmsd_rows.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64,
+                                          ctypes.c_int64, _f64p, _f64p]
+        lib.oracle_crmsd_rows.restype = None
+        lib.oracle_crmsd_pairs.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, _i64p, _i64p,
+                                           ctypes.c_int64, _f64p, _f64p]
+        lib.oracle_crmsd_pairs.restype = None
+        lib.oracle_crmsd_one_vs_all.argtypes = [_f32p, _f32p, ctypes.c_int64, ctypes.c_int32, _f64p, _f64p]
+        lib.oracle_crmsd_one_vs_all.restype = None
+        lib.oracle_num_threads.restype = ctypes.c_int
+        lib.oracle_set_num_threads.argtypes = [ctypes.c_int]
+        _lib = lib
+    return _lib
+
+
+def _f32(x, shape_tail=None):
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    return x
+
+
+def _p(a, t):
+    return a.ctypes.data_as(t)
+
+
+def num_threads() -> int:
+    return int(_load().oracle_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    _load().oracle_set_num_threads(int(n))
+
+
+def center(coords):
+    """coords[N][L][3] fp32 -> (centred[N][L][3] fp64, r2[N] fp64).  Steps 1-2."""
+    x = _f32(coords)
+    N, L, _ = x.shape
+    cen = np.empty((N, L, 3), np.float64)
+    r2 = np.empty(N, np.float64)
+    _load().oracle_center(_p(x, _f32p), N, L, _p(cen, _f64p), _p(r2, _f64p))
+    return cen, r2
+
+
+def crmsd_pair(xa, xb):
+    """(c, c2) of one pair by the definition route (centre, covariance, Jacobi SVD, sign det)."""
+    a, b = _f32(xa), _f32(xb)
+    assert a.shape == b.shape and a.shape[1] == 3
+    c2 = ctypes.c_double()
+    c = _load().oracle_crmsd_pair(_p(a, _f32p), _p(b, _f32p), a.shape[0], ctypes.byref(c2))
+    return float(c), float(c2.value)
+
+
+def crmsd_pair_eq2(xa, xb):
+    """eq. 2 literally: returns (c, c2, lambdas[3] of M^T M descending, S)."""
+    a, b = _f32(xa), _f32(xb)
+    c2 = ctypes.c_double()
+    S = ctypes.c_double()
+    lam = np.empty(3, np.float64)
+    c = _load().oracle_crmsd_pair_eq2(_p(a, _f32p), _p(b, _f32p), a.shape[0], ctypes.byref(c2),
+                                      _p(lam, _f64p), ctypes.byref(S))
+    return float(c), float(c2.value), lam, float(S.value)
+
+
+def crmsd_pair_eq1(xa, xb):
+    """eq. 1 literally: explicit optimal rotation, residual summed per atom.  (c, c2, R[3][3])."""
+    a, b = _f32(xa), _f32(xb)
+    c2 = ctypes.c_double()
+    R = np.empty((3, 3), np.float64)
+    c = _load().oracle_crmsd_pair_eq1(_p(a, _f32p), _p(b, _f32p), a.shape[0], ctypes.byref(c2),
+                                      _p(R, _f64p))
+    return float(c), float(c2.value), R
+
+
+def pair_spectrum(xa, xb):
+    """(singular values of M descending, det M, M[3][3]) of one pair."""
+    a, b = _f32(xa), _f32(xb)
+    s = np.empty(3, np.float64)
+    M = np.empty((3, 3), np.float64)
+    d = ctypes.c_double()
+    _load().oracle_pair_spectrum(_p(a, _f32p), _p(b, _f32p), a.shape[0], _p(s, _f64p), ctypes.byref(d),
+                                 _p(M, _f64p))
+    return s, float(d.value), M
+
+
+def crmsd_rows(coords, row_begin, row_end):
+    """Rows [row_begin,row_end) of the packed all-vs-all matrix: (c, c2) fp64, row-major, j>i."""
+    x = _f32(coords)
+    N, L, _ = x.shape
+    n = (row_begin * (2 * N - row_begin - 1) // 2, row_end * (2 * N - row_end - 1) // 2)
+    c = np.empty(n[1] - n[0], np.float64)
+    c2 = np.empty(n[1] - n[0], np.float64)
+    _load().oracle_crmsd_rows(_p(x, _f32p), N, L, int(row_begin), int(row_end), _p(c, _f64p), _p(c2, _f64p))
+    return c, c2
+
+
+def crmsd_allpairs(coords):
+    """Whole packed upper triangle, N(N-1)/2 values: (c, c2) fp64."""
+    x = _f32(coords)
+    return crmsd_rows(x, 0, x.shape[0])
+
+
+def crmsd_pairs(coords, pi, pj):
+    """Listed pairs: (c, c2) with c[k] = cRMSD(model pi[k], model pj[k])."""
+    x = _f32(coords)
+    N, L, _ = x.shape
+    pi = np.ascontiguousarray(pi, np.int64)
+    pj = np.ascontiguousarray(pj, np.int64)
+    c = np.empty(pi.size, np.float64)
+    c2 = np.empty(pi.size, np.float64)
+    _load().oracle_crmsd_pairs(_p(x, _f32p), N, L, _p(pi, _i64p), _p(pj, _i64p), pi.size,
+                               _p(c, _f64p), _p(c2, _f64p))
+    return c, c2
+
+
+def crmsd_one_vs_all(native, coords):
+    """One native[L][3] against coords[N][L][3]: (c, c2) fp64."""
+    nat = _f32(native)
+    x = _f32(coords)
+    N, L, _ = x.shape
+    assert nat.shape == (L, 3)
+    c = np.empty(N, np.float64)
+    c2 = np.empty(N, np.float64)
+    _load().oracle_crmsd_one_vs_all(_p(nat, _f32p), _p(x, _f32p), N, L, _p(c, _f64p), _p(c2, _f64p))
+    return c, c2
