@@ -1,0 +1,287 @@
+#!/usr/bin/env python
+"""bench.py -- all-vs-all cRMSD throughput on BASELINE.json's headline config (C3: N=10000, L=250).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload C3] [--engine auto]
+
+A step = one pass of the whole hot path (centring + R^2, covariance/Gram, eq. 2 closed form, packed
+store) over one synthetic decoy ensemble already resident in HBM.  Prints ONE JSON line (rank 0).
+`--impl reference` times the FP64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "all-vs-all cRMSD pairs/sec"
+UNIT = "pairs/s"
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=d["hbm_gbs"], bf16_tflops=d["bf16_tflops"], sm_max_mhz=d.get("sm_max_mhz", 1965.0),
+                    source="measured")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.index), "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = float(r[1])
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(ens, seconds: float = 15.0):
+    """Time the FP64 oracle, as it stands, on the first R rows of the ensemble (about `seconds` of CPU)."""
+    import oracle
+    N = ens.N
+    t0 = time.perf_counter()
+    c, _ = oracle.crmsd_rows(ens.coords, 0, 2)
+    probe_rows = 2
+    dt = time.perf_counter() - t0
+    rate = c.size / max(dt, 1e-6)                      # includes centring all N models once
+    t0 = time.perf_counter()
+    c, _ = oracle.crmsd_rows(ens.coords, 0, 8)
+    dt = time.perf_counter() - t0
+    rate = max(rate, c.size / max(dt, 1e-6))
+    rows = int(min(N - 1, max(8, seconds * rate / N)))
+    t0 = time.perf_counter()
+    c, _ = oracle.crmsd_rows(ens.coords, 0, rows)
+    dt = time.perf_counter() - t0
+    del probe_rows
+    return dict(value=c.size / dt, unit=UNIT, cores=oracle.num_threads(), kind="oracle",
+                sample=f"rows 0..{rows - 1} of {ens.name} ({c.size} pairs, {dt:.1f} s wall; FP64 Jacobi-SVD per pair, "
+                       f"OpenMP over rows; centring of all {N} models included)"), c.size, dt
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    from paper_1302_4000_b200 import workloads as wl
+    ens = wl.make_config(args.workload)
+    per_step_s = max(2.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_sample(ens, per_step_s)
+    tot_pairs, tot_t, last = 0, 0.0, None
+    for _ in range(args.steps):
+        last, n, dt = oracle_sample(ens, per_step_s)
+        tot_pairs += n
+        tot_t += dt
+    value = tot_pairs / tot_t
+    last["value"] = value
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: N={ens.N} models x L={ens.L} C-alpha, all-vs-all",
+                   "sample": last["sample"]},
+        "cpu_baseline": last,
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C1", "C2", "C3", "C4"])
+    ap.add_argument("--engine", default="auto", choices=["auto", "ffma", "i8tc"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import numpy as np
+    import torch
+    import paper_1302_4000_b200 as clusco
+    from paper_1302_4000_b200 import workloads as wl
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    clusco.load()
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    engine = {"auto": clusco.ENGINE_AUTO, "ffma": clusco.ENGINE_FFMA, "i8tc": clusco.ENGINE_I8TC}[args.engine]
+    # one independent ensemble per rank (the paper clusters 56 targets independently):
+    # rank r perturbs nothing but owns its own copy of the workload -> weak scaling, no collective.
+    ens = wl.make_config(args.workload)
+    N, L = ens.N, ens.L
+    P = N * (N - 1) // 2
+    if engine == clusco.ENGINE_AUTO:
+        engine = clusco.ENGINE_I8TC if clusco.engine_supported(clusco.ENGINE_I8TC, L) else clusco.ENGINE_FFMA
+    coords = torch.from_numpy(ens.coords).cuda()
+    out = torch.empty(P, dtype=torch.float32, device="cuda")
+    ws = torch.empty(clusco.clusco_crmsd_allpairs_workspace(N, L), dtype=torch.uint8, device="cuda")
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")       # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step(mid=None):
+        # the whole hot path = clusco_crmsd_allpairs, issued as its two stages so that an event between
+        # them isolates the dominant (fused Gram + eq. 2 + store) kernel inside the timed region
+        clusco.clusco_allpairs_prepare(coords, ws, engine)
+        if mid is not None:
+            mid.record(stream)
+        clusco.clusco_allpairs_compute(N, L, out, ws, engine)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev = [tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    for a, m, b in ev:
+        flush.zero_()                                   # L2 flush between timed iterations (untimed)
+        a.record(stream)
+        step(m)
+        b.record(stream)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    total_ms = sum(a.elapsed_time(b) for a, m, b in ev)
+    kern_ms = sum(m.elapsed_time(b) for a, m, b in ev) / args.steps
+    clocks = sampler.stop() if rank == 0 else None
+    if dist:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * P / (ms_per_step * 1e-3)
+
+    # e2e: the host-buffer C-ABI call, host<->device copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        h_in = torch.from_numpy(ens.coords).pin_memory()
+        h_out = torch.empty(P, dtype=torch.float32).pin_memory()
+        clusco.clusco_crmsd_allpairs_host(h_in, h_out)
+        reps = max(2, min(args.steps, 5))
+        if dist:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            clusco.clusco_crmsd_allpairs_host(h_in, h_out)
+        dt = (time.perf_counter() - t0) / reps
+        if dist:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * P / dt, "unit": UNIT, "h2d_bytes_per_step": int(N * L * 12),
+               "d2h_bytes_per_step": int(P * 4), "ms_per_step": dt * 1e3}
+
+    if rank != 0:
+        if dist:
+            dist.destroy_process_group()
+        return
+
+    # roofline for the dominant kernel (the fused Gram+epilogue kernel): algorithmic flops 18*L per pair
+    pk = _peaks()
+    flops = 18.0 * L * P
+    if engine == clusco.ENGINE_FFMA:
+        peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12          # FP32 FFMA: #SM x 128 lanes x 2 x clock
+        roof = {"bound": "alu", "achieved": flops / (kern_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                "peak_source": "148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz (DESIGN.md)"}
+    else:
+        peak = 2.0 * pk["bf16_tflops"]                                # int8 dense = 2x bf16 (nominal ratio)
+        roof = {"bound": "tensor", "achieved": flops / (kern_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                "peak_source": f"2 x {pk['source']} bf16 burst peak (int8:bf16 nominal ratio)"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["kernel_ms"] = kern_ms
+    roof["kernel"] = "gram_ffma_kernel" if engine == clusco.ENGINE_FFMA else "gram_i8tc_kernel"
+    roof["hbm_bound_ms"] = (4.0 * P + 12.0 * N * L) / (pk["hbm_gbs"] * 1e9) * 1e3
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        cpu, _, _ = oracle_sample(ens, 15.0)
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f32" if engine == clusco.ENGINE_FFMA else "s8 x s8 -> s32 (3x8-bit fixed point), f32 epilogue",
+        "data": "synthetic",
+        "config": {"workload": f"{args.workload}: N={N} models x L={L} C-alpha, all-vs-all packed upper triangle "
+                               f"({P} pairs), one ensemble per GPU",
+                   "engine": {1: "ffma", 2: "i8tc"}[engine], "l2": "flushed between timed iterations (256 MB write)",
+                   "effective_tflops": flops * world / (ms_per_step * 1e-3) / 1e12},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step(engine) * args.steps,
+        "roofline": roof, "cpu_baseline": cpu,
+    }))
+    if dist:
+        dist.destroy_process_group()
+
+
+def launches_per_step(engine):
+    return 3     # model_stats_kernel, operand-plane kernel, fused Gram+epilogue kernel
+
+
+if __name__ == "__main__":
+    main()

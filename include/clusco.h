@@ -1,0 +1,135 @@
+/*
+ * clusco.h -- C ABI of the B200-native (sm_100a) cRMSD library.
+ *
+ * The calls follow the problem statement of the ClusCo paper (arxiv 1302.4000; citations are
+ * /root/reference/PAPER.md:<line>): an ensemble of N models of L C-alpha atoms each, equal length
+ * and one-to-one atom correspondence (eq. 1 has a single atom index i), is compared
+ * all-versus-all -- N(N-1)/2 scores -- or against one reference/native structure
+ * (PAPER.md:84, 126-134).  The score is the coordinate RMSD after optimal superposition (eq. 1),
+ * obtained WITHOUT a rotation matrix from the 3x3 covariance matrix M of the pair, the eigenvalues of
+ * M^T M found as cubic roots, S = sign det M and the two radii of gyration (eq. 2):
+ *
+ *     cRMSD = sqrt( R_A^2 + R_B^2 - 2 (sqrt(l1) + sqrt(l2) + S sqrt(l3)) ).
+ *
+ * Conventions for every call
+ *   - Pointers are DEVICE pointers unless the name ends in _host.  The caller owns every buffer; the
+ *     library keeps no reference after the call is enqueued and frees nothing of the caller's.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Device-pointer
+ *     calls are asynchronous on that stream and never synchronise the device.  *_host calls block.
+ *   - coords[N][L][3]: float32, row-major, xyz interleaved, Angstrom (any unit; the result is in the
+ *     same unit).  Need not be centred.  Base pointers must be 16-byte aligned.
+ *   - Return value: clusco_status (0 = OK).  Nothing throws or aborts across the ABI.
+ *     N < 0, L < 1, or a NULL pointer with a non-empty extent -> CLUSCO_ERR_INVALID_ARG.
+ *     N == 0 (or N < 2 for all-pairs) is valid and writes nothing.
+ *   - NaN/Inf coordinates propagate to NaN results for the pairs they touch (no error: the call is
+ *     asynchronous).  Results are symmetric by construction; the diagonal is not stored.
+ *   - A device that is not compute capability 10.x -> CLUSCO_ERR_UNSUPPORTED_DEVICE.  There is no
+ *     CPU fallback.
+ */
+#ifndef CLUSCO_H
+#define CLUSCO_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    CLUSCO_OK = 0,
+    CLUSCO_ERR_INVALID_ARG = 1,
+    CLUSCO_ERR_WORKSPACE_TOO_SMALL = 2,
+    CLUSCO_ERR_UNSUPPORTED_DEVICE = 3,
+    CLUSCO_ERR_CUDA = 4
+} clusco_status;
+
+/* Gram-stage engines of the all-pairs kernel.                              */
+typedef enum {
+    CLUSCO_ENGINE_AUTO = 0,   /* the library's default for this device and shape                      */
+    CLUSCO_ENGINE_FFMA = 1,   /* fp32 CUDA-core Gram, 16-atom blocked accumulation                    */
+    CLUSCO_ENGINE_I8TC = 2    /* tcgen05 kind::i8 tensor-core Gram on 3x8-bit fixed-point slices,
+                                 exact int32 accumulation in TMEM                                     */
+} clusco_engine;
+
+/* Static, never freed. */
+const char* clusco_status_string(int status);
+/* cudaError_t behind the last CLUSCO_ERR_CUDA returned on this host thread (0 if none). */
+int clusco_last_cuda_error(void);
+/* Library version, "major.minor". */
+const char* clusco_version(void);
+
+/* 1 if `engine` can run models of L atoms on the current build, else 0 (host-only query). */
+int clusco_engine_supported(int engine, int32_t L);
+
+/*
+ * Centring and radius of gyration (implicit in eq. 2: M and R are taken about the centroid,
+ * PAPER.md:40-45).   coords[N][L][3] -> centred[N][L][3] = x_i - mean(x)   (same layout; may alias
+ * coords; may be NULL), r2[N] = (1/L) sum_i |x_i - mean|^2 = R^2 (may be NULL).
+ */
+int clusco_center(const float* coords, int64_t N, int32_t L, float* centred, float* r2, void* stream);
+
+/*
+ * Workspace for the all-pairs call: bytes of device scratch (operand planes in the Gram stage's
+ * layout + per-model scale and sum of squares).  Returns 0 for invalid arguments.
+ */
+size_t clusco_crmsd_allpairs_workspace(int64_t N, int32_t L);
+
+/*
+ * All-versus-all cRMSD (eq. 2 for every pair; N(N-1)/2 values).
+ *   out[N(N-1)/2]: row-major packed upper triangle, for i < j
+ *       out[ i*(2N-i-1)/2 + (j-i-1) ] = cRMSD(model i, model j).
+ *   workspace: >= clusco_crmsd_allpairs_workspace(N, L) bytes, 256-byte aligned, contents undefined
+ *       on entry and exit; else CLUSCO_ERR_WORKSPACE_TOO_SMALL.
+ */
+int clusco_crmsd_allpairs(const float* coords, int64_t N, int32_t L, float* out,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * The same with an explicit Gram engine and a row range: computes rows [row_begin, row_end) of the
+ * packed triangle -- the contiguous slice
+ *       out_rows[ idx(i,j) - idx(row_begin, row_begin+1) ],  row_begin <= i < row_end, j > i
+ * -- so that ranks of a multi-GPU job each own one contiguous slice of the matrix and exchange
+ * nothing.  row_begin must be a multiple of 128 (or 0) unless row_begin == row_end.
+ */
+int clusco_crmsd_allpairs_ex(const float* coords, int64_t N, int32_t L,
+                             int64_t row_begin, int64_t row_end, float* out_rows,
+                             void* workspace, size_t workspace_bytes, int engine, void* stream);
+
+/*
+ * The two stages of the all-pairs call, separately (clusco_crmsd_allpairs_ex = prepare + compute on one
+ * stream).  prepare: steps a1+a2 -- centroid, power-of-two scale and sum of squares per model, and the
+ * operand planes of `engine` -- written into `workspace`.  compute: steps a3-a5 for rows
+ * [row_begin,row_end) from a prepared workspace (same N, L, engine; AUTO resolves identically in both).
+ * A prepared workspace can serve any number of compute calls (row ranges, repeated timing).
+ */
+int clusco_allpairs_prepare(const float* coords, int64_t N, int32_t L, void* workspace,
+                            size_t workspace_bytes, int engine, void* stream);
+int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out_rows,
+                            void* workspace, size_t workspace_bytes, int engine, void* stream);
+
+/*
+ * One reference structure against N models: native[L][3], coords[N][L][3]
+ * (neither pre-centred) -> out[N], out[k] = cRMSD(native, model k).
+ */
+int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L,
+                            float* out, void* stream);
+
+/*
+ * Host-buffer convenience calls (blocking): allocate device memory, copy in, compute, copy the
+ * result back, free.  coords_host / out_host are ordinary (preferably pinned) host pointers.
+ */
+int clusco_crmsd_allpairs_host(const float* coords_host, int64_t N, int32_t L, float* out_host);
+int clusco_crmsd_one_vs_all_host(const float* native_host, const float* coords_host, int64_t N,
+                                 int32_t L, float* out_host);
+
+/*
+ * Balanced row partition for `parts` ranks: writes parts+1 boundaries (multiples of 128, first 0,
+ * last N) such that each [b[r], b[r+1]) owns about the same number of pairs.  Host-only arithmetic.
+ */
+int clusco_partition_rows(int64_t N, int32_t parts, int64_t* boundaries_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CLUSCO_H */

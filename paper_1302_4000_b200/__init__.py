@@ -1,0 +1,220 @@
+"""paper_1302_4000_b200 -- B200-native (sm_100a) cRMSD: thin Python binding over the C ABI in include/clusco.h.
+
+Argument marshalling only: every step of the path (centring, covariance/Gram, the eq. 2 closed form,
+packed store, one-vs-all) runs in the CUDA kernels of `csrc/`, reached through `libclusco.so`.
+PyTorch is used for device memory and streams, nothing else.  There is NO CPU fallback: if the library
+is missing or the device is not a B200-class GPU the calls raise.
+
+    import paper_1302_4000_b200 as clusco
+    out = clusco.clusco_crmsd_allpairs(coords)            # coords: cuda float32 [N, L, 3] -> [N(N-1)/2]
+    d   = clusco.clusco_crmsd_one_vs_all(native, coords)  # -> [N]
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libclusco.so")
+_lib = None
+
+ENGINE_AUTO, ENGINE_FFMA, ENGINE_I8TC = 0, 1, 2
+
+EXPORTS = (
+    "clusco_status_string", "clusco_last_cuda_error", "clusco_version", "clusco_center",
+    "clusco_crmsd_allpairs_workspace", "clusco_crmsd_allpairs", "clusco_crmsd_allpairs_ex",
+    "clusco_crmsd_one_vs_all", "clusco_crmsd_allpairs_host", "clusco_crmsd_one_vs_all_host",
+    "clusco_partition_rows", "clusco_engine_supported", "clusco_allpairs_prepare", "clusco_allpairs_compute",
+)
+
+
+class CluscoError(RuntimeError):
+    pass
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load(build_if_missing: bool = False):
+    """dlopen libclusco.so (built in-tree by `python -m paper_1302_4000_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        if not build_if_missing:
+            raise CluscoError(f"{_LIB_PATH} is missing: run `python -m paper_1302_4000_b200.build` "
+                              "(there is no CPU fallback)")
+        from . import build as _build
+        _build.build()
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, i64, i32, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_size_t
+    lib.clusco_status_string.argtypes = [ctypes.c_int]
+    lib.clusco_status_string.restype = ctypes.c_char_p
+    lib.clusco_last_cuda_error.restype = ctypes.c_int
+    lib.clusco_version.restype = ctypes.c_char_p
+    lib.clusco_center.argtypes = [vp, i64, i32, vp, vp, vp]
+    lib.clusco_crmsd_allpairs_workspace.argtypes = [i64, i32]
+    lib.clusco_crmsd_allpairs_workspace.restype = sz
+    lib.clusco_crmsd_allpairs.argtypes = [vp, i64, i32, vp, vp, sz, vp]
+    lib.clusco_crmsd_allpairs_ex.argtypes = [vp, i64, i32, i64, i64, vp, vp, sz, ctypes.c_int, vp]
+    lib.clusco_crmsd_one_vs_all.argtypes = [vp, vp, i64, i32, vp, vp]
+    lib.clusco_crmsd_allpairs_host.argtypes = [vp, i64, i32, vp]
+    lib.clusco_crmsd_one_vs_all_host.argtypes = [vp, vp, i64, i32, vp]
+    lib.clusco_partition_rows.argtypes = [i64, i32, ctypes.POINTER(ctypes.c_int64)]
+    lib.clusco_engine_supported.argtypes = [ctypes.c_int, i32]
+    lib.clusco_allpairs_prepare.argtypes = [vp, i64, i32, vp, sz, ctypes.c_int, vp]
+    lib.clusco_allpairs_compute.argtypes = [i64, i32, i64, i64, vp, vp, sz, ctypes.c_int, vp]
+    for name in EXPORTS:                       # every declared symbol must be exported
+        getattr(lib, name)
+    _lib = lib
+    return lib
+
+
+def _check(status: int, what: str):
+    if status != 0:
+        lib = load()
+        msg = lib.clusco_status_string(status).decode()
+        extra = f" (cudaError {lib.clusco_last_cuda_error()})" if status == 4 else ""
+        raise CluscoError(f"{what}: {msg}{extra}")
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _stream_ptr(t):
+    torch = _torch()
+    return ctypes.c_void_p(torch.cuda.current_stream(t.device).cuda_stream)
+
+
+def _ptr(t):
+    return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
+
+
+def _check_coords(coords, name="coords"):
+    torch = _torch()
+    if not (isinstance(coords, torch.Tensor) and coords.is_cuda and coords.dtype == torch.float32
+            and coords.dim() == 3 and coords.shape[2] == 3 and coords.is_contiguous()):
+        raise CluscoError(f"{name} must be a contiguous CUDA float32 tensor of shape [N, L, 3]")
+    return int(coords.shape[0]), int(coords.shape[1])
+
+
+def version() -> str:
+    return load().clusco_version().decode()
+
+
+def engine_supported(engine: int, L: int) -> bool:
+    return bool(load().clusco_engine_supported(engine, L))
+
+
+def n_pairs(N: int) -> int:
+    return N * (N - 1) // 2
+
+
+def clusco_center(coords, centred=None, r2=None):
+    """coords[N][L][3] -> (centred[N][L][3], r2[N]); see include/clusco.h."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    if centred is None:
+        centred = torch.empty_like(coords)
+    if r2 is None:
+        r2 = torch.empty(N, dtype=torch.float32, device=coords.device)
+    with torch.cuda.device(coords.device):
+        _check(load().clusco_center(_ptr(coords), N, L, _ptr(centred), _ptr(r2), _stream_ptr(coords)),
+               "clusco_center")
+    return centred, r2
+
+
+def clusco_crmsd_allpairs_workspace(N: int, L: int) -> int:
+    return int(load().clusco_crmsd_allpairs_workspace(N, L))
+
+
+def clusco_crmsd_allpairs(coords, out=None, workspace=None, engine: int = ENGINE_AUTO,
+                          row_begin: int = 0, row_end: int | None = None):
+    """All-versus-all cRMSD: packed upper triangle float32[N(N-1)/2] (rows [row_begin,row_end) if given)."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    row_end = N if row_end is None else row_end
+    lo = row_begin * (2 * N - row_begin - 1) // 2
+    hi = row_end * (2 * N - row_end - 1) // 2
+    if out is None:
+        out = torch.empty(max(hi - lo, 0), dtype=torch.float32, device=coords.device)
+    nbytes = clusco_crmsd_allpairs_workspace(N, L)
+    if workspace is None:
+        workspace = torch.empty(nbytes, dtype=torch.uint8, device=coords.device)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_crmsd_allpairs_ex(_ptr(coords), N, L, row_begin, row_end, _ptr(out), _ptr(workspace),
+                                             workspace.numel() * workspace.element_size(), engine,
+                                             _stream_ptr(coords))
+    _check(st, "clusco_crmsd_allpairs")
+    return out
+
+
+def clusco_allpairs_prepare(coords, workspace, engine: int = ENGINE_AUTO):
+    """Stage 1 of the all-pairs call (centring, R^2, operand planes) into `workspace`."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_allpairs_prepare(_ptr(coords), N, L, _ptr(workspace),
+                                            workspace.numel() * workspace.element_size(), engine,
+                                            _stream_ptr(coords))
+    _check(st, "clusco_allpairs_prepare")
+
+
+def clusco_allpairs_compute(N: int, L: int, out, workspace, engine: int = ENGINE_AUTO, row_begin: int = 0,
+                            row_end: int | None = None):
+    """Stage 2 of the all-pairs call (Gram + eq. 2 + packed store) from a prepared workspace."""
+    torch = _torch()
+    row_end = N if row_end is None else row_end
+    with torch.cuda.device(out.device):
+        st = load().clusco_allpairs_compute(N, L, row_begin, row_end, _ptr(out), _ptr(workspace),
+                                            workspace.numel() * workspace.element_size(), engine,
+                                            _stream_ptr(out))
+    _check(st, "clusco_allpairs_compute")
+    return out
+
+
+def clusco_crmsd_one_vs_all(native, coords, out=None):
+    """One native[L][3] against coords[N][L][3] -> float32[N]."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    if not (native.is_cuda and native.dtype == torch.float32 and tuple(native.shape) == (L, 3)
+            and native.is_contiguous()):
+        raise CluscoError("native must be a contiguous CUDA float32 tensor of shape [L, 3]")
+    if out is None:
+        out = torch.empty(N, dtype=torch.float32, device=coords.device)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_crmsd_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
+    _check(st, "clusco_crmsd_one_vs_all")
+    return out
+
+
+def clusco_crmsd_allpairs_host(coords_host, out_host=None):
+    """Host-buffer call (blocking): CPU float32 tensors in and out; copies are inside the call."""
+    torch = _torch()
+    assert coords_host.dtype == torch.float32 and not coords_host.is_cuda and coords_host.is_contiguous()
+    N, L = int(coords_host.shape[0]), int(coords_host.shape[1])
+    if out_host is None:
+        out_host = torch.empty(n_pairs(N), dtype=torch.float32, pin_memory=True)
+    _check(load().clusco_crmsd_allpairs_host(_ptr(coords_host), N, L, _ptr(out_host)),
+           "clusco_crmsd_allpairs_host")
+    return out_host
+
+
+def clusco_crmsd_one_vs_all_host(native_host, coords_host, out_host=None):
+    torch = _torch()
+    N, L = int(coords_host.shape[0]), int(coords_host.shape[1])
+    if out_host is None:
+        out_host = torch.empty(N, dtype=torch.float32, pin_memory=True)
+    _check(load().clusco_crmsd_one_vs_all_host(_ptr(native_host), _ptr(coords_host), N, L, _ptr(out_host)),
+           "clusco_crmsd_one_vs_all_host")
+    return out_host
+
+
+def clusco_partition_rows(N: int, parts: int):
+    """Row boundaries (multiples of 128) giving each of `parts` ranks about the same number of pairs."""
+    b = (ctypes.c_int64 * (parts + 1))()
+    _check(load().clusco_partition_rows(N, parts, b), "clusco_partition_rows")
+    return [int(v) for v in b]

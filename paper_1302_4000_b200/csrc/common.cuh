@@ -1,0 +1,72 @@
+// common.cuh -- shared host/device helpers of libclusco (no arithmetic of the method lives here).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/clusco.h"
+
+namespace clusco {
+
+// ---- per-model record produced by the stats kernel and consumed by every Gram engine -------------
+// The centred coordinates of model n are scaled by 2^-ex so that max |a| lies in [0.5, 1); S = sum of
+// squares of the scaled fp32 values (accumulated in FP64, stored as a two-float sum Shi + Slo).
+struct ModelStat {
+    double mean[3];
+    float Shi, Slo;
+    int32_t ex;
+    int32_t pad;
+};
+
+static inline int64_t round_up(int64_t a, int64_t b) { return (a + b - 1) / b * b; }
+
+// thread-local last CUDA error for clusco_last_cuda_error()
+extern thread_local int g_last_cuda_error;
+
+#define CLUSCO_CUDA_TRY(expr)                                   \
+    do {                                                        \
+        cudaError_t _e = (expr);                                \
+        if (_e != cudaSuccess) {                                \
+            ::clusco::g_last_cuda_error = (int)_e;              \
+            return CLUSCO_ERR_CUDA;                             \
+        }                                                       \
+    } while (0)
+
+// packed row-major upper-triangle index of (i, j), i < j  (N(N-1)/2 values)
+__host__ __device__ __forceinline__ int64_t packed_index(int64_t i, int64_t j, int64_t N)
+{
+    return i * (2 * N - i - 1) / 2 + (j - i - 1);
+}
+
+// exact 2^k as float for k in [-126, 127]
+__device__ __forceinline__ float pow2i(int k) { return __int_as_float((k + 127) << 23); }
+
+// ---- workspace layout --------------------------------------------------------------------------
+// [ ModelStat[Np] | engine operand planes ]      Np = N rounded up to 128
+struct Workspace {
+    int64_t N, Np;
+    int32_t L;
+    int32_t Lp16;        // L rounded up to 16 (FFMA k-chunk)
+    int32_t Lp32;        // L rounded up to 32 (kind::i8 MMA K)
+    size_t off_stats, off_ffma, off_i8, total;
+};
+
+static inline Workspace workspace_layout(int64_t N, int32_t L)
+{
+    Workspace w;
+    w.N = N;
+    w.L = L;
+    w.Np = round_up(N, 128);
+    w.Lp16 = (int32_t)round_up(L, 16);
+    w.Lp32 = (int32_t)round_up(L, 32);
+    size_t o = 0;
+    w.off_stats = o;
+    o += (size_t)round_up((int64_t)sizeof(ModelStat) * w.Np, 256);
+    w.off_ffma = o;                                        // float Yt[Lp16][3*Np]
+    o += (size_t)round_up((int64_t)sizeof(float) * w.Lp16 * 3 * w.Np, 256);
+    w.off_i8 = o;                                          // int8 slices, see gram_i8tc.cuh
+    o += (size_t)round_up((int64_t)3 * 3 * w.Np * w.Lp32, 256);
+    w.total = o;
+    return w;
+}
+
+}  // namespace clusco

@@ -1,0 +1,226 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element.
+
+Tolerance (BASELINE.json north_star): for EVERY pair |c^2_gpu - c^2_oracle| <= 2e-3 A^2, and
+|c_gpu - c_oracle| <= 1e-3 A wherever c_oracle >= 0.5 A.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1302_4000_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_C2 = 2e-3
+TOL_C = 1e-3
+
+
+@pytest.fixture(scope="module")
+def clusco():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: -m gpu tests need the B200 box")
+    import paper_1302_4000_b200 as pkg
+    pkg.load()                                   # fails loudly if libclusco.so is missing
+    return pkg
+
+
+def _dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def _engines(clusco, L):
+    eng = [clusco.ENGINE_FFMA]
+    if clusco.engine_supported(clusco.ENGINE_I8TC, L):
+        eng.append(clusco.ENGINE_I8TC)
+    return eng
+
+
+def assert_parity(c_gpu, c_ref, c2_ref, what=""):
+    c_gpu = np.asarray(c_gpu, np.float64)
+    assert c_gpu.shape == c_ref.shape, (what, c_gpu.shape, c_ref.shape)
+    assert np.all(np.isfinite(c_gpu)), what
+    d2 = np.abs(c_gpu * c_gpu - c2_ref)
+    k = int(np.argmax(d2)) if d2.size else 0
+    assert d2.size == 0 or d2[k] <= TOL_C2, f"{what}: max |dc2| {d2[k]:.3e} at {k} (c_ref {c_ref[k]:.6f})"
+    big = c_ref >= 0.5
+    if big.any():
+        dc = np.abs(c_gpu - c_ref)[big]
+        assert dc.max() <= TOL_C, f"{what}: max |dc| {dc.max():.3e} over c>=0.5"
+    return float(d2.max()) if d2.size else 0.0
+
+
+# ---- a1 + a2 -----------------------------------------------------------------------------------------
+
+def test_center_matches_oracle(clusco, c1):
+    cen, r2 = clusco.clusco_center(_dev(c1.coords))
+    cen_o, r2_o = oracle.center(c1.coords)
+    assert np.max(np.abs(cen.cpu().numpy().astype(np.float64) - cen_o)) <= 8e-6      # half an fp32 ulp at 64..128 A
+    assert np.max(np.abs(r2.cpu().numpy() / r2_o - 1.0)) <= 2e-7
+    # in place, and with either output omitted
+    x = _dev(c1.coords).clone()
+    clusco.clusco_center(x, centred=x)
+    assert np.array_equal(x.cpu().numpy(), cen.cpu().numpy())
+
+
+# ---- a3..a5 all-pairs: whole configs the oracle finishes in seconds ----------------------------------
+
+@pytest.mark.parametrize("cfg,N", [("C1", None), ("C2", None), ("C3", 1200), ("C4", 1500)])
+def test_allpairs_every_pair(clusco, cfg, N):
+    ens = wl.make_config(cfg, N=N)
+    c_ref, c2_ref = oracle.crmsd_allpairs(ens.coords)
+    for eng in _engines(clusco, ens.L):
+        out = clusco.clusco_crmsd_allpairs(_dev(ens.coords), engine=eng).cpu().numpy()
+        worst = assert_parity(out, c_ref, c2_ref, f"{cfg} engine {eng}")
+        print(f"{cfg} N={ens.N} L={ens.L} engine={eng}: max|dc2| = {worst:.2e}")
+
+
+def test_allpairs_C1_specials(clusco, c1):
+    out = clusco.clusco_crmsd_allpairs(_dev(c1.coords)).cpu().numpy()
+    a, b = sorted(int(v) for v in c1.rigid_copy_idx)
+    assert out[wl.packed_index(a, b, c1.N)] < 0.05              # rigid copies: c ~ 1e-5, c^2 tolerance applies
+    for m in c1.mirror_idx:                                      # mirrors keep chirality (S = -1): far from 0
+        i, j = sorted((int(m), a))
+        assert out[wl.packed_index(i, j, c1.N)] > 1.0
+
+
+# ---- full-size configs in the launch configuration bench.py times: sampled outputs --------------------
+
+@pytest.mark.parametrize("cfg", ["C3", "C4"])
+def test_allpairs_full_size_sampled(clusco, cfg):
+    ens = wl.make_config(cfg)
+    N = ens.N
+    rng = np.random.default_rng(99)
+    out = clusco.clusco_crmsd_allpairs(_dev(ens.coords))
+    assert out.numel() == N * (N - 1) // 2
+    # (i) random pairs, (ii) whole rows incl. first / last / tile-boundary rows
+    pi = rng.integers(0, N, 200_000)
+    pj = rng.integers(0, N, 200_000)
+    keep = pi != pj
+    pi, pj = np.minimum(pi, pj)[keep], np.maximum(pi, pj)[keep]
+    rows = [0, 1, 127, 128, 129, N // 2, N - 130, N - 2] + list(rng.integers(0, N - 1, 8))
+    for r in rows:
+        pi = np.concatenate([pi, np.full(N - 1 - r, r)])
+        pj = np.concatenate([pj, np.arange(r + 1, N)])
+    c_ref, c2_ref = oracle.crmsd_pairs(ens.coords, pi, pj)
+    import torch
+    idx = torch.from_numpy(wl.packed_index(pi, pj, N)).cuda()
+    got = out[idx].cpu().numpy()
+    worst = assert_parity(got, c_ref, c2_ref, f"{cfg} full size")
+    print(f"{cfg} full size, {len(pi)} sampled pairs: max|dc2| = {worst:.2e}")
+    # properties that hold at any size: finite, within the bounds (R_A-R_B)^2 <= c^2 <= R_A^2+R_B^2
+    assert bool(torch.isfinite(out).all())
+    _, r2 = oracle.center(ens.coords)
+    assert float(out.max()) ** 2 <= 2 * r2.max() + 1e-2
+
+
+# ---- ragged shapes, tile edges, degenerate inputs -----------------------------------------------------
+
+@pytest.mark.parametrize("N,L", [(2, 5), (3, 1), (5, 2), (31, 15), (33, 16), (64, 17), (129, 33), (257, 76),
+                                 (300, 250), (130, 887)])
+def test_allpairs_ragged_shapes(clusco, N, L):
+    rng = np.random.default_rng(1000 * N + L)
+    nat = wl.random_walk_chain(L, rng)
+    y = nat[None] + rng.normal(size=(N, L, 3)) * rng.uniform(0.0, 3.0, size=(N, 1, 1))
+    x = wl.rigid_transform(y, rng).astype(np.float32)
+    c_ref, c2_ref = oracle.crmsd_allpairs(x)
+    for eng in _engines(clusco, L):
+        out = clusco.clusco_crmsd_allpairs(_dev(x), engine=eng).cpu().numpy()
+        assert_parity(out, c_ref, c2_ref, f"N={N} L={L} engine {eng}")
+
+
+def test_allpairs_empty_and_single(clusco):
+    import torch
+    for N in (0, 1):
+        x = torch.zeros((N, 7, 3), dtype=torch.float32, device="cuda")
+        assert clusco.clusco_crmsd_allpairs(x).numel() == 0
+
+
+def test_allpairs_degenerate_models(clusco):
+    rng = np.random.default_rng(5)
+    L = 40
+    base = wl.random_walk_chain(L, rng)
+    line = np.stack([np.linspace(0, 60, L), np.zeros(L), np.zeros(L)], 1)            # collinear: rank-1 M
+    plane = base * np.array([1.0, 1.0, 0.0])                                         # planar: det M = 0
+    point = np.zeros((L, 3)) + 7.0                                                   # all atoms coincide: M = 0
+    models = [base, base.copy(), base * np.array([-1.0, 1, 1]), line, line * 1.5, plane,
+              plane * np.array([-1.0, 1, 1]), point, base * 2.0]
+    x = wl.rigid_transform(np.array(models), rng).astype(np.float32)
+    c_ref, c2_ref = oracle.crmsd_allpairs(x)
+    for eng in _engines(clusco, L):
+        out = clusco.clusco_crmsd_allpairs(_dev(x), engine=eng).cpu().numpy()
+        assert_parity(out, c_ref, c2_ref, f"degenerate, engine {eng}")
+
+
+def test_nan_propagates_to_its_pairs_only(clusco, c1):
+    x = c1.coords[:40].copy()
+    x[7, 3, 1] = np.nan
+    out = clusco.clusco_crmsd_allpairs(_dev(x)).cpu().numpy()
+    iu = np.triu_indices(40, 1)
+    touched = (iu[0] == 7) | (iu[1] == 7)
+    assert np.all(np.isnan(out[touched])) and np.all(np.isfinite(out[~touched]))
+
+
+def test_allpairs_row_ranges_are_slices(clusco):
+    ens = wl.make_config("C2", N=700)
+    x = _dev(ens.coords)
+    full = clusco.clusco_crmsd_allpairs(x).cpu().numpy()
+    N = ens.N
+    bounds = [0, 128, 384, 640, N]
+    parts = [clusco.clusco_crmsd_allpairs(x, row_begin=lo, row_end=hi).cpu().numpy()
+             for lo, hi in zip(bounds, bounds[1:])]
+    assert np.array_equal(np.concatenate(parts), full)
+
+
+def test_allpairs_host_call(clusco, c1):
+    import torch
+    out = clusco.clusco_crmsd_allpairs_host(torch.from_numpy(c1.coords))
+    ref = clusco.clusco_crmsd_allpairs(_dev(c1.coords)).cpu()
+    assert torch.equal(out, ref)
+
+
+# ---- a6 one-vs-all --------------------------------------------------------------------------------------
+
+def test_one_vs_all_prefix(clusco):
+    ens = wl.make_config("C5", N=20_000, chunk=100_000)
+    c_ref, c2_ref = oracle.crmsd_one_vs_all(ens.native, ens.coords)
+    out = clusco.clusco_crmsd_one_vs_all(_dev(ens.native), _dev(ens.coords)).cpu().numpy()
+    worst = assert_parity(out, c_ref, c2_ref, "C5 prefix")
+    print(f"C5 20000-model prefix: max|dc2| = {worst:.2e}")
+
+
+@pytest.mark.parametrize("N,L", [(1, 3), (31, 2), (33, 150), (1000, 37), (77, 887)])
+def test_one_vs_all_ragged(clusco, N, L):
+    rng = np.random.default_rng(7 * N + L)
+    nat = wl.random_walk_chain(L, rng)
+    y = nat[None] + rng.normal(size=(N, L, 3)) * rng.uniform(0.0, 4.0, size=(N, 1, 1))
+    y[0] = nat
+    if N > 2:
+        y[2] = nat * np.array([-1.0, 1.0, 1.0])
+    x = wl.rigid_transform(y, rng).astype(np.float32)
+    nat32 = wl.rigid_transform(nat[None], rng)[0].astype(np.float32)
+    c_ref, c2_ref = oracle.crmsd_one_vs_all(nat32, x)
+    out = clusco.clusco_crmsd_one_vs_all(_dev(nat32), _dev(x)).cpu().numpy()
+    assert_parity(out, c_ref, c2_ref, f"one-vs-all N={N} L={L}")
+
+
+def test_one_vs_all_full_size_sampled(clusco):
+    import torch
+    N, chunk = 1_000_000, 100_000
+    ens0 = wl.make_config("C5", N=N, chunk=chunk, chunks=range(0))
+    coords = torch.empty((N, 150, 3), dtype=torch.float32, device="cuda")
+    keep = {}
+    for k in range(N // chunk):
+        part = wl.make_config("C5", N=N, chunk=chunk, chunks=range(k, k + 1))
+        coords[k * chunk:(k + 1) * chunk] = torch.from_numpy(part.coords).cuda()
+        if k in (0, 4, 9):
+            keep[k] = part.coords
+    out = clusco.clusco_crmsd_one_vs_all(_dev(ens0.native), coords)
+    assert bool(torch.isfinite(out).all())
+    for k, x in keep.items():
+        c_ref, c2_ref = oracle.crmsd_one_vs_all(ens0.native, x[:20_000])
+        got = out[k * chunk:k * chunk + 20_000].cpu().numpy()
+        assert_parity(got, c_ref, c2_ref, f"C5 full size chunk {k}")
+    out_h = clusco.clusco_crmsd_one_vs_all_host(torch.from_numpy(ens0.native), torch.from_numpy(keep[0][:5000]))
+    assert torch.equal(out_h, out[:5000].cpu())
