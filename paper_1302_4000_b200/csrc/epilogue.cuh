@@ -23,6 +23,15 @@ namespace clusco {
 
 struct EPair { float E0; float delta; };
 
+// a*b - c*d with one rounding error of the result (Kahan): w = c*d rounded, e = exact error of w
+__device__ __forceinline__ float diff_of_products(float a, float b, float c, float d)
+{
+    const float w = c * d;
+    const float e = fmaf(-c, d, w);
+    const float f = fmaf(a, b, -w);
+    return f + e;
+}
+
 __device__ __forceinline__ EPair eq2_energy(const float m[9])
 {
     // c2 = |M|_F^2
@@ -30,17 +39,19 @@ __device__ __forceinline__ EPair eq2_energy(const float m[9])
 #pragma unroll
     for (int i = 1; i < 9; ++i) c2 = fmaf(m[i], m[i], c2);
 
-    // cofactor rows: C0 = r1 x r2, C1 = r2 x r0, C2 = r0 x r1
+    // cofactor rows: C0 = r1 x r2, C1 = r2 x r0, C2 = r0 x r1.  Each entry is a difference of products
+    // evaluated with Kahan's FMA scheme (error ~1 ulp of the result): for a rank-deficient M the cofactors
+    // are pure cancellation, and det M below inherits their relative accuracy.
     float C[9];
-    C[0] = fmaf(m[4], m[8], -m[5] * m[7]);
-    C[1] = fmaf(m[5], m[6], -m[3] * m[8]);
-    C[2] = fmaf(m[3], m[7], -m[4] * m[6]);
-    C[3] = fmaf(m[7], m[2], -m[8] * m[1]);
-    C[4] = fmaf(m[8], m[0], -m[6] * m[2]);
-    C[5] = fmaf(m[6], m[1], -m[7] * m[0]);
-    C[6] = fmaf(m[1], m[5], -m[2] * m[4]);
-    C[7] = fmaf(m[2], m[3], -m[0] * m[5]);
-    C[8] = fmaf(m[0], m[4], -m[1] * m[3]);
+    C[0] = diff_of_products(m[4], m[8], m[5], m[7]);
+    C[1] = diff_of_products(m[5], m[6], m[3], m[8]);
+    C[2] = diff_of_products(m[3], m[7], m[4], m[6]);
+    C[3] = diff_of_products(m[7], m[2], m[8], m[1]);
+    C[4] = diff_of_products(m[8], m[0], m[6], m[2]);
+    C[5] = diff_of_products(m[6], m[1], m[7], m[0]);
+    C[6] = diff_of_products(m[1], m[5], m[2], m[4]);
+    C[7] = diff_of_products(m[2], m[3], m[0], m[5]);
+    C[8] = diff_of_products(m[0], m[4], m[1], m[3]);
     float c1 = C[0] * C[0];
 #pragma unroll
     for (int i = 1; i < 9; ++i) c1 = fmaf(C[i], C[i], c1);
