@@ -40,14 +40,29 @@ __host__ __device__ __forceinline__ int64_t packed_index(int64_t i, int64_t j, i
 // exact 2^k as float for k in [-126, 127]
 __device__ __forceinline__ float pow2i(int k) { return __int_as_float((k + 127) << 23); }
 
+// compact per-model record read by the epilogues with one 16-byte load
+struct __align__(16) PairStat {
+    float Shi, Slo;     // two-float sum of squares of the scaled coordinates (engine units)
+    int32_t ex;         // scale exponent
+    int32_t pad;
+};
+
+// ---- tensor-core engine geometry (gram_i8tc.cuh) ---------------------------------------------------
+constexpr int I8_ROW_MODELS = 40;      // models per row tile: 4 TMEM quadrants x (10 models x 3 comps + 2 zero rows)
+constexpr int I8_COL_MODELS = 16;      // models per column tile: MMA N = 3 x 16 = 48 per level block
+constexpr int I8_A_SLAB = 128 * 32;    // bytes of one (k-step, slice) A slab: 128 rows x 32 atoms, int8
+constexpr int I8_B_SLAB = 144 * 32;    // bytes of one k-step B slab: 3 slices x 48 rows x 32 atoms
+constexpr int I8_MAX_KSTEPS = 8;       // L <= 256: A tile resident in shared memory, int32 level sums cannot overflow
+
 // ---- workspace layout --------------------------------------------------------------------------
-// [ ModelStat[Np] | engine operand planes ]      Np = N rounded up to 128
+// [ ModelStat[Np] | PairStat[Np] | FFMA plane | i8 A planes | i8 B planes ]      Np = N rounded up to 128
 struct Workspace {
     int64_t N, Np;
     int32_t L;
     int32_t Lp16;        // L rounded up to 16 (FFMA k-chunk)
     int32_t Lp32;        // L rounded up to 32 (kind::i8 MMA K)
-    size_t off_stats, off_ffma, off_i8, total;
+    int64_t row_tiles, col_tiles;   // i8 engine
+    size_t off_stats, off_pstat, off_ffma, off_i8a, off_i8b, total;
 };
 
 static inline Workspace workspace_layout(int64_t N, int32_t L)
@@ -58,13 +73,20 @@ static inline Workspace workspace_layout(int64_t N, int32_t L)
     w.Np = round_up(N, 128);
     w.Lp16 = (int32_t)round_up(L, 16);
     w.Lp32 = (int32_t)round_up(L, 32);
+    w.row_tiles = (N + I8_ROW_MODELS - 1) / I8_ROW_MODELS;
+    w.col_tiles = (N + I8_COL_MODELS - 1) / I8_COL_MODELS;
     size_t o = 0;
     w.off_stats = o;
     o += (size_t)round_up((int64_t)sizeof(ModelStat) * w.Np, 256);
+    w.off_pstat = o;
+    o += (size_t)round_up((int64_t)sizeof(PairStat) * w.Np, 256);
     w.off_ffma = o;                                        // float Yt[Lp16][3*Np]
     o += (size_t)round_up((int64_t)sizeof(float) * w.Lp16 * 3 * w.Np, 256);
-    w.off_i8 = o;                                          // int8 slices, see gram_i8tc.cuh
-    o += (size_t)round_up((int64_t)3 * 3 * w.Np * w.Lp32, 256);
+    const int64_t ks = w.Lp32 / 32;
+    w.off_i8a = o;                                         // int8 Ap[row_tiles][ks][3][I8_A_SLAB]
+    o += (size_t)round_up(w.row_tiles * ks * 3 * I8_A_SLAB, 256);
+    w.off_i8b = o;                                         // int8 Bp[col_tiles][ks][I8_B_SLAB]
+    o += (size_t)round_up(w.col_tiles * ks * I8_B_SLAB, 256);
     w.total = o;
     return w;
 }
