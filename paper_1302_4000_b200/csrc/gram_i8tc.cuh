@@ -1,21 +1,407 @@
-// gram_i8tc.cuh -- tensor-core engine of the all-pairs kernel (tcgen05 kind::i8).  Placeholder until the
-// kernel lands: reports "unsupported" so AUTO falls back to the FFMA engine.
+// gram_i8tc.cuh -- tensor-core engine of the all-pairs kernel: steps a3 (covariance), a4 (eq. 2 closed form) and
+// a5 (packed store) fused in one persistent, warp-specialised kernel on tcgen05 (kind::i8) with int32
+// accumulators in TMEM.
+//
+// Arithmetic: the centred coordinates of model n, scaled by 2^-ex_n so that max|a| is in
+// [0.5, 1), are multiplied by KAPPA 2^23 (KAPPA = 127/128) and rounded to a 24-bit integer
+//      I = d0 2^16 + d1 2^8 + d2,        d0, d1, d2 signed 8-bit digits (|d0| <= 127 thanks to KAPPA).
+// The nine covariance sums of a pair are then  G = sum_k I_A I_B = 2^32 V0 + 2^24 V1 + 2^16 V2 (+ two
+// dropped low-order levels),  V0 = d0.d0,  V1 = d0.d1 + d1.d0,  V2 = d0.d2 + d1.d1 + d2.d0: six int8 products,
+// accumulated EXACTLY in int32.  The sums of squares of eq. 2's R^2 are taken from the same integers.
+//
+// Tile = 32 row models x 16 column models.  MMA view: A = [128 rows x K] with row (= TMEM lane) 32 w + 8 p + r
+// holding component p of row model 8 w + r (p = 3: zero rows), B = [48 rows x K] per digit with row 16 q + o
+// holding component q of column model (o & 1) * 4 + ((o >> 1) & 3) + (o & 8).  Per 32-atom k-step three MMAs
+//      D[  0:144) += A(d0) . [B(d0); B(d1); B(d2)]^T      (levels 0, 1, 2)
+//      D[ 48:144) += A(d1) . [B(d0); B(d1)]^T              (levels 1, 2)
+//      D[ 96:144) += A(d2) . [B(d0)]^T                     (level 2)
+// leave level v of (p, q, pair) at TMEM column 48 v + 16 q + o.  With this placement a 16x256b TMEM load hands
+// every epilogue thread the three components p of ONE row model (lanes r, r+8, r+16) for two column models, so
+// the nine sums of a pair meet in one thread without any shuffle.
+//
+// Roles: warp 0 = bulk-copy producer (operand planes are stored in HBM as shared-memory images in the
+// canonical K-major core-matrix layout, so tiles arrive by plain 1-D cp.async.bulk), warp 1 = MMA issuer
+// (one thread) and TMEM owner, warps 2..17 = two epilogue teams of 8 warps (4 TMEM quadrants x 2 column
+// halves) that alternate over tiles; three TMEM accumulator buffers of 144 columns.
 #pragma once
 #include "common.cuh"
+#include "epilogue.cuh"
+#include "tc_ptx.cuh"
 
 namespace clusco {
 
-static inline bool i8tc_supported(int32_t) { return false; }
+constexpr double I8_KAPPA = 127.0 / 128.0;
+constexpr int I8_STAGES = 12;                  // B k-step slabs in flight
+constexpr int I8_ACC_COLS = 144;               // TMEM columns per accumulator buffer (3 levels x 48)
+constexpr int I8_ACC_BUFS = 3;
+constexpr int I8_EPI_WARPS = 16;
+constexpr int I8_THREADS = (2 + I8_EPI_WARPS) * 32;
 
-static inline int i8tc_prepare(const float*, int64_t, int32_t, const Workspace&, char*, ModelStat*, cudaStream_t)
+static inline bool i8tc_supported(int32_t L) { return L >= 1 && L <= 32 * I8_MAX_KSTEPS; }
+
+// ---- operand planes ---------------------------------------------------------------------------------------
+// Ap[row_tile][digit][kstep][I8_A_SLAB], Bp[col_tile][kstep][I8_B_SLAB]; a slab is a grid of 8-row x 16-byte core
+// matrices: byte (row, k) of a slab sits at (row/8)*256 + (k/16)*128 + (row%8)*16 + k%16.
+// One warp per model slot; lane = atom within the k-step.
+__global__ void __launch_bounds__(256) i8_plane_kernel(const float* __restrict__ coords, int64_t N, int32_t L,
+                                                       int32_t ks, int64_t row_slots, int64_t col_slots,
+                                                       int64_t stat_slots, const ModelStat* __restrict__ stats,
+                                                       int8_t* __restrict__ Ap, int8_t* __restrict__ Bp,
+                                                       PairStat* __restrict__ pstat)
 {
-    return CLUSCO_ERR_INVALID_ARG;
+    const int lane = threadIdx.x & 31;
+    const int64_t n = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (n >= stat_slots) return;
+    const bool valid = n < N;
+    double mean[3] = {0.0, 0.0, 0.0};
+    double scale = 0.0;
+    int ex = 0;
+    if (valid) {
+        const ModelStat s = stats[n];
+        mean[0] = s.mean[0]; mean[1] = s.mean[1]; mean[2] = s.mean[2];
+        ex = s.ex;
+        scale = ldexp(I8_KAPPA, 23 - ex);
+    }
+    const float* x = coords + n * (int64_t)L * 3;
+    // A image: row tile n/32, quadrant w = (n%32)/8, row-in-group r = n%8, row group 4w + p
+    const int64_t a_tile = n >> 5;
+    const int a_w = (int)(n & 31) >> 3, a_r = (int)(n & 7);
+    // B image: column tile n/16, o = position of this model among the 16 columns of a component block
+    const int64_t b_tile = n >> 4;
+    const int m16 = (int)(n & 15);
+    const int b_o = (m16 & 8) | ((m16 & 3) << 1) | ((m16 >> 2) & 1);
+    const int kc = lane >> 4, kb = lane & 15;
+    unsigned long long sumsq = 0ull;
+    bool finite = true;
+    for (int kk = 0; kk < ks; ++kk) {
+        const int k = kk * 32 + lane;
+#pragma unroll
+        for (int p = 0; p < 3; ++p) {
+            int I = 0;
+            if (valid && k < L) {
+                const float xv = x[3 * k + p];
+                finite = finite && (fabsf(xv) <= 3.0e38f);
+                I = __double2int_rn(((double)xv - mean[p]) * scale);
+            }
+            sumsq += (unsigned long long)((long long)I * (long long)I);
+            const int d2 = (int)(int8_t)(I & 0xff);
+            const int I1 = (I - d2) >> 8;
+            const int d1 = (int)(int8_t)(I1 & 0xff);
+            const int d0 = (I1 - d1) >> 8;
+            const int8_t dig[3] = {(int8_t)d0, (int8_t)d1, (int8_t)d2};
+            if (n < row_slots) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+                    Ap[((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + p) * 256 + kc * 128 + a_r * 16 + kb] = dig[a];
+            }
+            if (n < col_slots) {
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+                    Bp[(b_tile * ks + kk) * I8_B_SLAB + b * 1536 + (2 * p + (b_o >> 3)) * 256 + kc * 128 + (b_o & 7) * 16 + kb] =
+                        dig[b];
+            }
+        }
+        if (n < row_slots) {                               // the zero rows (p = 3) of this model's quadrant
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                Ap[((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + 3) * 256 + kc * 128 + a_r * 16 + kb] = 0;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sumsq += __shfl_xor_sync(0xffffffffu, sumsq, o);
+    finite = __all_sync(0xffffffffu, finite);
+    if (lane == 0) {
+        const double S = (double)sumsq * 0x1p-46;          // units: (KAPPA 2^-ex)^2 Angstrom^2
+        PairStat ps;
+        ps.Shi = (float)S;
+        ps.Slo = (float)(S - (double)ps.Shi);
+        if (!finite) ps.Shi = __int_as_float(0x7fc00000);  // NaN/Inf coordinates poison this model's pairs
+        ps.ex = ex;
+        ps.pad = 0;
+        pstat[n] = ps;
+    }
 }
 
-static inline int i8tc_compute(int64_t, int32_t, int64_t, int64_t, float*, const Workspace&, char*, ModelStat*, int,
-                               cudaStream_t)
+// ---- tile walk ----------------------------------------------------------------------------------------------
+// Row tile I (32 models) meets column tiles J = 2I .. Tc-1 (16 models each).  Tiles of the call's row-tile range
+// [I_lo, I_hi) are linearised row-major; CTA b owns the contiguous range [total b / G, total (b+1) / G).
+struct I8Tiles {
+    int64_t Tc, I_lo, I_hi, total;
+};
+__host__ __device__ __forceinline__ int64_t i8_tiles_before(const I8Tiles& t, int64_t I)
 {
-    return CLUSCO_ERR_INVALID_ARG;
+    return (I - t.I_lo) * t.Tc - (I * (I - 1) - t.I_lo * (t.I_lo - 1));
+}
+__device__ __forceinline__ void i8_tile_from_linear(const I8Tiles& t, int64_t lin, int64_t& I, int64_t& J)
+{
+    int64_t lo = t.I_lo, hi = t.I_hi - 1;                  // largest I with tiles_before(I) <= lin
+    while (lo < hi) {
+        const int64_t mid = (lo + hi + 1) >> 1;
+        if (i8_tiles_before(t, mid) <= lin) lo = mid; else hi = mid - 1;
+    }
+    I = lo;
+    J = 2 * I + (lin - i8_tiles_before(t, I));
+}
+
+struct I8Params {
+    const int8_t* Ap;
+    const int8_t* Bp;
+    const PairStat* pstat;
+    float* out;
+    int64_t N, row_begin, row_end, base;
+    int32_t ks;
+    int32_t wide;          // 1: level sums may exceed the int32 combine (L > 250) -> combine in fp32
+    float invLk;           // 1 / (KAPPA^2 L)
+    I8Tiles tiles;
+};
+
+__global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params P)
+{
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int ks = P.ks;
+    uint8_t* sA = smem;                                          // 3 digits x ks x 4096
+    uint8_t* sB = smem + (size_t)3 * ks * I8_A_SLAB;             // I8_STAGES x 4608
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)I8_STAGES * I8_B_SLAB);
+    // barrier map: [0,S) b_full, [S,2S) b_empty, 2S a_full, 2S+1 a_empty, 2S+2.. acc_full[3], acc_empty[3]
+    const uint32_t bar0 = ptx::smem_u32(bars);
+    auto B_FULL = [&](int s) { return bar0 + 8u * s; };
+    auto B_EMPTY = [&](int s) { return bar0 + 8u * (I8_STAGES + s); };
+    const uint32_t A_FULL = bar0 + 8u * (2 * I8_STAGES), A_EMPTY = A_FULL + 8u;
+    auto ACC_FULL = [&](int b) { return bar0 + 8u * (2 * I8_STAGES + 2 + b); };
+    auto ACC_EMPTY = [&](int b) { return bar0 + 8u * (2 * I8_STAGES + 2 + I8_ACC_BUFS + b); };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * I8_STAGES + 2 + 2 * I8_ACC_BUFS);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < I8_STAGES; ++s) {
+            ptx::mbar_init(B_FULL(s), 1);
+            ptx::mbar_init(B_EMPTY(s), 1);
+        }
+        ptx::mbar_init(A_FULL, 1);
+        ptx::mbar_init(A_EMPTY, 1);
+        for (int b = 0; b < I8_ACC_BUFS; ++b) {
+            ptx::mbar_init(ACC_FULL(b), 1);
+            ptx::mbar_init(ACC_EMPTY(b), I8_EPI_WARPS / 2);
+        }
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    const int64_t G = gridDim.x, b = blockIdx.x;
+    const int64_t t0 = P.tiles.total * b / G, t1 = P.tiles.total * (b + 1) / G;
+    const int64_t Tc = P.tiles.Tc;
+
+    if (warp == 0) {
+        // ===== producer =====
+        if (lane == 0) {
+            int64_t I, J;
+            i8_tile_from_linear(P.tiles, t0, I, J);
+            int64_t curI = -1;
+            uint32_t a_loads = 0, stage = 0, phase = 0;
+            for (int64_t t = t0; t < t1; ++t) {
+                if (I != curI) {
+                    ptx::mbar_wait(A_EMPTY, (a_loads & 1) ^ 1);
+                    ptx::mbar_expect_tx(A_FULL, 3u * ks * I8_A_SLAB);
+                    const int8_t* src = P.Ap + (size_t)I * 3 * ks * I8_A_SLAB;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+                        ptx::bulk_g2s(ptx::smem_u32(sA + (size_t)a * ks * I8_A_SLAB), src + (size_t)a * ks * I8_A_SLAB,
+                                      (uint32_t)ks * I8_A_SLAB, A_FULL);
+                    ++a_loads;
+                    curI = I;
+                }
+                const int8_t* srcB = P.Bp + (size_t)J * ks * I8_B_SLAB;
+                for (int kk = 0; kk < ks; ++kk) {
+                    ptx::mbar_wait(B_EMPTY(stage), phase ^ 1);
+                    ptx::mbar_expect_tx(B_FULL(stage), I8_B_SLAB);
+                    ptx::bulk_g2s(ptx::smem_u32(sB + (size_t)stage * I8_B_SLAB), srcB + (size_t)kk * I8_B_SLAB, I8_B_SLAB,
+                                  B_FULL(stage));
+                    if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
+                }
+                if (++J >= Tc) { ++I; J = 2 * I; }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer =====
+        if (lane == 0) {
+            int64_t I, J;
+            i8_tile_from_linear(P.tiles, t0, I, J);
+            int64_t curI = -1;
+            uint32_t a_uses = 0, stage = 0, phase = 0, n = 0;
+            constexpr uint32_t ID144 = ptx::idesc_s8(128, 144), ID96 = ptx::idesc_s8(128, 96), ID48 = ptx::idesc_s8(128, 48);
+            const uint32_t sA_u = ptx::smem_u32(sA), sB_u = ptx::smem_u32(sB);
+            for (int64_t t = t0; t < t1; ++t, ++n) {
+                if (I != curI) {
+                    ptx::mbar_wait(A_FULL, a_uses & 1);
+                    ++a_uses;
+                    curI = I;
+                }
+                const uint32_t buf = n % I8_ACC_BUFS;
+                ptx::mbar_wait(ACC_EMPTY(buf), ((n / I8_ACC_BUFS) & 1) ^ 1);
+                ptx::tc_fence_after();
+                const uint32_t d = tmem + buf * I8_ACC_COLS;
+                for (int kk = 0; kk < ks; ++kk) {
+                    ptx::mbar_wait(B_FULL(stage), phase);
+                    ptx::tc_fence_after();
+                    const uint64_t db = ptx::smem_desc(sB_u + stage * I8_B_SLAB, 128, 256);
+                    const uint64_t da0 = ptx::smem_desc(sA_u + (0 * ks + kk) * I8_A_SLAB, 128, 256);
+                    const uint64_t da1 = ptx::smem_desc(sA_u + (1 * ks + kk) * I8_A_SLAB, 128, 256);
+                    const uint64_t da2 = ptx::smem_desc(sA_u + (2 * ks + kk) * I8_A_SLAB, 128, 256);
+                    ptx::mma_i8(d, da0, db, ID144, kk > 0);
+                    ptx::mma_i8(d + 48, da1, db, ID96, 1);
+                    ptx::mma_i8(d + 96, da2, db, ID48, 1);
+                    ptx::tc_commit(B_EMPTY(stage));
+                    if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
+                }
+                ptx::tc_commit(ACC_FULL(buf));
+                if (++J >= Tc) { ++I; J = 2 * I; }
+                if (I != curI || t + 1 == t1) ptx::tc_commit(A_EMPTY);
+            }
+        }
+    } else {
+        // ===== epilogue =====
+        const int ew = warp - 2;
+        const int team = ew >> 3, half = (ew & 7) >> 2;          // column half: models 8*half .. 8*half+7 of the tile
+        const int quad = warp & 3;                               // TMEM lanes 32 quad .. 32 quad + 31
+        const int r = lane >> 2, c4 = lane & 3;
+        int64_t I, J;
+        i8_tile_from_linear(P.tiles, t0 + team, I, J);
+        for (int64_t t = t0 + team, n = team; t < t1; t += 2, n += 2) {
+            const uint32_t buf = (uint32_t)(n % I8_ACC_BUFS);
+            ptx::mbar_wait(ACC_FULL(buf), (uint32_t)((n / I8_ACC_BUFS) & 1));
+            ptx::tc_fence_after();
+            const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16) + buf * I8_ACC_COLS + half * 8;
+            // m[e][3p+q]: pair (row model r, column model c4 + 4e + 8 half)
+            float m[2][9];
+            {
+                uint32_t v1[3][2][4], v2[3][2][4];
+#pragma unroll
+                for (int q = 0; q < 3; ++q)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 48 + 16 * q, v1[q][h]);
+                        ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 96 + 16 * q, v2[q][h]);
+                    }
+                ptx::tmem_ld_wait();
+                if (!P.wide) {
+                    int32_t T[2][9];
+#pragma unroll
+                    for (int q = 0; q < 3; ++q)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            T[e][0 + q] = ((int32_t)v1[q][0][e] << 8) + (int32_t)v2[q][0][e];
+                            T[e][3 + q] = ((int32_t)v1[q][0][2 + e] << 8) + (int32_t)v2[q][0][2 + e];
+                            T[e][6 + q] = ((int32_t)v1[q][1][e] << 8) + (int32_t)v2[q][1][e];
+                        }
+#pragma unroll
+                    for (int e = 0; e < 2; ++e)
+#pragma unroll
+                        for (int i = 0; i < 9; ++i) m[e][i] = (float)T[e][i] * 0x1p-30f;
+                } else {
+#pragma unroll
+                    for (int q = 0; q < 3; ++q)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            m[e][0 + q] = fmaf((float)(int32_t)v1[q][0][e], 0x1p-22f, (float)(int32_t)v2[q][0][e] * 0x1p-30f);
+                            m[e][3 + q] = fmaf((float)(int32_t)v1[q][0][2 + e], 0x1p-22f, (float)(int32_t)v2[q][0][2 + e] * 0x1p-30f);
+                            m[e][6 + q] = fmaf((float)(int32_t)v1[q][1][e], 0x1p-22f, (float)(int32_t)v2[q][1][e] * 0x1p-30f);
+                        }
+                }
+            }
+            {
+                uint32_t v0[3][2][4];
+#pragma unroll
+                for (int q = 0; q < 3; ++q)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 16 * q, v0[q][h]);
+                ptx::tmem_ld_wait();
+#pragma unroll
+                for (int q = 0; q < 3; ++q)
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        m[e][0 + q] = fmaf((float)(int32_t)v0[q][0][e], 0x1p-14f, m[e][0 + q]);
+                        m[e][3 + q] = fmaf((float)(int32_t)v0[q][0][2 + e], 0x1p-14f, m[e][3 + q]);
+                        m[e][6 + q] = fmaf((float)(int32_t)v0[q][1][e], 0x1p-14f, m[e][6 + q]);
+                    }
+            }
+            // the accumulator buffer is free again
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
+
+            const int64_t i = I * I8_ROW_MODELS + quad * 8 + r;
+            if (i < P.N && i >= P.row_begin && i < P.row_end) {
+                const PairStat si = P.pstat[i];
+                const int64_t rowoff = i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int64_t j = J * I8_COL_MODELS + half * 8 + 4 * e + c4;
+                    if (j < P.N && j > i) {
+                        const PairStat sj = P.pstat[j];
+                        P.out[rowoff + j] = eq2_crmsd(m[e], si.Shi, si.Slo, si.ex, sj.Shi, sj.Slo, sj.ex, P.invLk);
+                    }
+                }
+            }
+            // advance two tiles
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+                if (++J >= Tc) { ++I; J = 2 * I; }
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+}
+
+static inline size_t i8tc_smem_bytes(int ks)
+{
+    return (size_t)3 * ks * I8_A_SLAB + (size_t)I8_STAGES * I8_B_SLAB + 8 * (2 * I8_STAGES + 2 + 2 * I8_ACC_BUFS) + 16;
+}
+
+static inline int i8tc_prepare(const float* coords, int64_t N, int32_t L, const Workspace& w, char* ws,
+                               ModelStat* stats, cudaStream_t s)
+{
+    if (!i8tc_supported(L)) return CLUSCO_ERR_INVALID_ARG;
+    const int ks = w.Lp32 / 32;
+    const int64_t row_slots = w.row_tiles * I8_ROW_MODELS, col_slots = w.col_tiles * I8_COL_MODELS;
+    i8_plane_kernel<<<(unsigned)((w.Np + 7) / 8), 256, 0, s>>>(coords, N, L, ks, row_slots, col_slots, w.Np, stats,
+                                                               (int8_t*)(ws + w.off_i8a), (int8_t*)(ws + w.off_i8b),
+                                                               (PairStat*)(ws + w.off_pstat));
+    CLUSCO_CUDA_TRY(cudaGetLastError());
+    return CLUSCO_OK;
+}
+
+static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out,
+                               const Workspace& w, char* ws, ModelStat*, int sms, cudaStream_t s)
+{
+    if (!i8tc_supported(L)) return CLUSCO_ERR_INVALID_ARG;
+    I8Params P;
+    P.Ap = (const int8_t*)(ws + w.off_i8a);
+    P.Bp = (const int8_t*)(ws + w.off_i8b);
+    P.pstat = (const PairStat*)(ws + w.off_pstat);
+    P.out = out;
+    P.N = N;
+    P.row_begin = row_begin;
+    P.row_end = row_end;
+    P.base = packed_index(row_begin, row_begin + 1, N);
+    P.ks = w.Lp32 / 32;
+    P.wide = L > 250 ? 1 : 0;
+    P.invLk = (float)(1.0 / (I8_KAPPA * I8_KAPPA * (double)L));
+    P.tiles.Tc = w.col_tiles;
+    P.tiles.I_lo = row_begin / I8_ROW_MODELS;
+    P.tiles.I_hi = (row_end + I8_ROW_MODELS - 1) / I8_ROW_MODELS;
+    P.tiles.total = i8_tiles_before(P.tiles, P.tiles.I_hi);
+    if (P.tiles.total <= 0) return CLUSCO_OK;
+    const size_t smem = i8tc_smem_bytes(P.ks);
+    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gram_i8tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t grid = P.tiles.total < sms ? P.tiles.total : sms;
+    gram_i8tc_kernel<<<(unsigned)grid, I8_THREADS, smem, s>>>(P);
+    CLUSCO_CUDA_TRY(cudaGetLastError());
+    return CLUSCO_OK;
 }
 
 }  // namespace clusco
