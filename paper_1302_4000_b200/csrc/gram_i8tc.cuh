@@ -171,7 +171,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     auto ACC_EMPTY = [&](int b) { return bar0 + 8u * (2 * I8_STAGES + 2 + I8_ACC_BUFS + b); };
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * I8_STAGES + 2 + 2 * I8_ACC_BUFS);
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
         for (int s = 0; s < I8_STAGES; ++s) {
             ptx::mbar_init(B_FULL(s), 1);
@@ -226,41 +226,48 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             }
         }
     } else if (warp == 1) {
-        // ===== MMA issuer =====
-        if (lane == 0) {
-            int64_t I, J;
-            i8_tile_from_linear(P.tiles, t0, I, J);
-            int64_t curI = -1;
-            uint32_t a_uses = 0, stage = 0, phase = 0, n = 0;
-            constexpr uint32_t ID144 = ptx::idesc_s8(128, 144), ID96 = ptx::idesc_s8(128, 96), ID48 = ptx::idesc_s8(128, 48);
-            const uint32_t sA_u = ptx::smem_u32(sA), sB_u = ptx::smem_u32(sB);
-            for (int64_t t = t0; t < t1; ++t, ++n) {
-                if (I != curI) {
-                    ptx::mbar_wait(A_FULL, a_uses & 1);
-                    ++a_uses;
-                    curI = I;
-                }
-                const uint32_t buf = n % I8_ACC_BUFS;
-                ptx::mbar_wait(ACC_EMPTY(buf), ((n / I8_ACC_BUFS) & 1) ^ 1);
+        // ===== MMA issuer: the whole warp walks the loop (warp-uniform control flow and addresses, so the
+        // descriptors live in uniform registers); one elected lane issues =====
+        int64_t I, J;
+        i8_tile_from_linear(P.tiles, t0, I, J);
+        int64_t curI = -1;
+        uint32_t a_uses = 0, stage = 0, phase = 0, n = 0;
+        constexpr uint32_t ID144 = ptx::idesc_s8(128, 144), ID96 = ptx::idesc_s8(128, 96), ID48 = ptx::idesc_s8(128, 48);
+        // descriptor = hi word (SBO 256 B, version 1) | lo word (LBO 128 B, start address >> 4)
+        constexpr uint64_t DESC_HI = (uint64_t)((256u >> 4) | (1u << 14)) << 32;
+        const uint32_t a_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sA) & 0x3FFFFu) >> 4);
+        const uint32_t b_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sB) & 0x3FFFFu) >> 4);
+        const uint32_t a_digit = (uint32_t)ks * (I8_A_SLAB >> 4);
+        for (int64_t t = t0; t < t1; ++t, ++n) {
+            if (I != curI) {
+                ptx::mbar_wait(A_FULL, a_uses & 1);
+                ++a_uses;
+                curI = I;
+            }
+            const uint32_t buf = n % I8_ACC_BUFS;
+            ptx::mbar_wait(ACC_EMPTY(buf), ((n / I8_ACC_BUFS) & 1) ^ 1);
+            const uint32_t d = tmem + buf * I8_ACC_COLS;
+            uint32_t a_lo = a_lo0;
+            for (int kk = 0; kk < ks; ++kk) {
+                ptx::mbar_wait(B_FULL(stage), phase);
                 ptx::tc_fence_after();
-                const uint32_t d = tmem + buf * I8_ACC_COLS;
-                for (int kk = 0; kk < ks; ++kk) {
-                    ptx::mbar_wait(B_FULL(stage), phase);
-                    ptx::tc_fence_after();
-                    const uint64_t db = ptx::smem_desc(sB_u + stage * I8_B_SLAB, 128, 256);
-                    const uint64_t da0 = ptx::smem_desc(sA_u + (0 * ks + kk) * I8_A_SLAB, 128, 256);
-                    const uint64_t da1 = ptx::smem_desc(sA_u + (1 * ks + kk) * I8_A_SLAB, 128, 256);
-                    const uint64_t da2 = ptx::smem_desc(sA_u + (2 * ks + kk) * I8_A_SLAB, 128, 256);
-                    ptx::mma_i8(d, da0, db, ID144, kk > 0);
-                    ptx::mma_i8(d + 48, da1, db, ID96, 1);
-                    ptx::mma_i8(d + 96, da2, db, ID48, 1);
+                if (ptx::elect_one()) {
+                    const uint64_t db = DESC_HI | (b_lo0 + stage * (I8_B_SLAB >> 4));
+                    ptx::mma_i8(d, DESC_HI | a_lo, db, ID144, kk > 0);
+                    ptx::mma_i8(d + 48, DESC_HI | (a_lo + a_digit), db, ID96, 1);
+                    ptx::mma_i8(d + 96, DESC_HI | (a_lo + 2 * a_digit), db, ID48, 1);
                     ptx::tc_commit(B_EMPTY(stage));
-                    if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
                 }
+                __syncwarp();
+                a_lo += I8_A_SLAB >> 4;
+                if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
+            }
+            if (++J >= Tc) { ++I; J = 2 * I; }
+            if (ptx::elect_one()) {
                 ptx::tc_commit(ACC_FULL(buf));
-                if (++J >= Tc) { ++I; J = 2 * I; }
                 if (I != curI || t + 1 == t1) ptx::tc_commit(A_EMPTY);
             }
+            __syncwarp();
         }
     } else {
         // ===== epilogue =====
