@@ -31,7 +31,9 @@
 namespace clusco {
 
 constexpr double I8_KAPPA = 127.0 / 128.0;
-constexpr int I8_STAGES = 12;                  // B k-step slabs in flight
+constexpr int I8_KC = 4;                      // k-steps per B stage: one barrier round trip (~100 cycles) per 12 MMAs
+constexpr int I8_STAGE_BYTES = I8_KC * I8_B_SLAB;
+constexpr int I8_MAX_STAGES = 8;               // B stages in flight: as many as shared memory holds, up to this
 constexpr int I8_ACC_COLS = 144;               // TMEM columns per accumulator buffer (3 levels x 48)
 constexpr int I8_ACC_BUFS = 3;
 constexpr int I8_EPI_WARPS = 16;
@@ -150,6 +152,7 @@ struct I8Params {
     float* out;
     int64_t N, row_begin, row_end, base;
     int32_t ks;
+    int32_t stages;        // B ring depth
     int32_t wide;          // 1: level sums may exceed the int32 combine (L > 250) -> combine in fp32
     float invLk;           // 1 / (KAPPA^2 L)
     I8Tiles tiles;
@@ -160,8 +163,9 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     extern __shared__ __align__(128) uint8_t smem[];
     const int ks = P.ks;
     uint8_t* sA = smem;                                          // 3 digits x ks x 4096
-    uint8_t* sB = smem + (size_t)3 * ks * I8_A_SLAB;             // I8_STAGES x 4608
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)I8_STAGES * I8_B_SLAB);
+    const int I8_STAGES = P.stages;
+    uint8_t* sB = smem + (size_t)3 * ks * I8_A_SLAB;             // stages x I8_KC x 4608
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)I8_STAGES * I8_STAGE_BYTES);
     // barrier map: [0,S) b_full, [S,2S) b_empty, 2S a_full, 2S+1 a_empty, 2S+2.. acc_full[3], acc_empty[3]
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto B_FULL = [&](int s) { return bar0 + 8u * s; };
@@ -215,10 +219,11 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                     curI = I;
                 }
                 const int8_t* srcB = P.Bp + (size_t)J * ks * I8_B_SLAB;
-                for (int kk = 0; kk < ks; ++kk) {
+                for (int k0 = 0; k0 < ks; k0 += I8_KC) {
+                    const uint32_t bytes = (uint32_t)min(I8_KC, ks - k0) * I8_B_SLAB;
                     ptx::mbar_wait(B_EMPTY(stage), phase ^ 1);
-                    ptx::mbar_expect_tx(B_FULL(stage), I8_B_SLAB);
-                    ptx::bulk_g2s(ptx::smem_u32(sB + (size_t)stage * I8_B_SLAB), srcB + (size_t)kk * I8_B_SLAB, I8_B_SLAB,
+                    ptx::mbar_expect_tx(B_FULL(stage), bytes);
+                    ptx::bulk_g2s(ptx::smem_u32(sB + (size_t)stage * I8_STAGE_BYTES), srcB + (size_t)k0 * I8_B_SLAB, bytes,
                                   B_FULL(stage));
                     if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
                 }
@@ -247,19 +252,25 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             const uint32_t buf = n % I8_ACC_BUFS;
             ptx::mbar_wait(ACC_EMPTY(buf), ((n / I8_ACC_BUFS) & 1) ^ 1);
             const uint32_t d = tmem + buf * I8_ACC_COLS;
-            uint32_t a_lo = a_lo0;
-            for (int kk = 0; kk < ks; ++kk) {
+            for (int k0 = 0; k0 < ks; k0 += I8_KC) {
                 ptx::mbar_wait(B_FULL(stage), phase);
                 ptx::tc_fence_after();
                 if (ptx::elect_one()) {
-                    const uint64_t db = DESC_HI | (b_lo0 + stage * (I8_B_SLAB >> 4));
-                    ptx::mma_i8(d, DESC_HI | a_lo, db, ID144, kk > 0);
-                    ptx::mma_i8(d + 48, DESC_HI | (a_lo + a_digit), db, ID96, 1);
-                    ptx::mma_i8(d + 96, DESC_HI | (a_lo + 2 * a_digit), db, ID48, 1);
+                    const uint32_t a_lo = a_lo0 + k0 * (I8_A_SLAB >> 4);
+                    const uint32_t b_lo = b_lo0 + stage * (I8_STAGE_BYTES >> 4);
+#pragma unroll
+                    for (int k = 0; k < I8_KC; ++k) {
+                        if (k0 + k < ks) {
+                            const uint64_t db = DESC_HI | (b_lo + k * (I8_B_SLAB >> 4));
+                            const uint32_t ak = a_lo + k * (I8_A_SLAB >> 4);
+                            ptx::mma_i8(d, DESC_HI | ak, db, ID144, (k0 + k) > 0);
+                            ptx::mma_i8(d + 48, DESC_HI | (ak + a_digit), db, ID96, 1);
+                            ptx::mma_i8(d + 96, DESC_HI | (ak + 2 * a_digit), db, ID48, 1);
+                        }
+                    }
                     ptx::tc_commit(B_EMPTY(stage));
                 }
                 __syncwarp();
-                a_lo += I8_A_SLAB >> 4;
                 if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
             }
             if (++J >= Tc) { ++I; J = 2 * I; }
@@ -364,9 +375,15 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
 }
 
-static inline size_t i8tc_smem_bytes(int ks)
+static inline size_t i8tc_smem_bytes(int ks, int stages)
 {
-    return (size_t)3 * ks * I8_A_SLAB + (size_t)I8_STAGES * I8_B_SLAB + 8 * (2 * I8_STAGES + 2 + 2 * I8_ACC_BUFS) + 16;
+    return (size_t)3 * ks * I8_A_SLAB + (size_t)stages * I8_STAGE_BYTES + 8 * (2 * stages + 2 + 2 * I8_ACC_BUFS) + 16;
+}
+static inline int i8tc_stages(int ks)
+{
+    int st = I8_MAX_STAGES;
+    while (st > 2 && i8tc_smem_bytes(ks, st) > 227 * 1024) --st;
+    return st;
 }
 
 static inline int i8tc_prepare(const float* coords, int64_t N, int32_t L, const Workspace& w, char* ws,
@@ -403,7 +420,8 @@ static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t 
     P.tiles.I_hi = (row_end + I8_ROW_MODELS - 1) / I8_ROW_MODELS;
     P.tiles.total = i8_tiles_before(P.tiles, P.tiles.I_hi);
     if (P.tiles.total <= 0) return CLUSCO_OK;
-    const size_t smem = i8tc_smem_bytes(P.ks);
+    P.stages = i8tc_stages(P.ks);
+    const size_t smem = i8tc_smem_bytes(P.ks, P.stages);
     CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gram_i8tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t grid = P.tiles.total < sms ? P.tiles.total : sms;
     gram_i8tc_kernel<<<(unsigned)grid, I8_THREADS, smem, s>>>(P);
