@@ -42,9 +42,9 @@ __device__ __forceinline__ float pow2i(int k) { return __int_as_float((k + 127) 
 
 // compact per-model record read by the epilogues with one 16-byte load
 struct __align__(16) PairStat {
-    float Shi, Slo;     // two-float sum of squares of the scaled coordinates (engine units)
-    int32_t ex;         // scale exponent
-    int32_t pad;
+    float Thi, Tlo;     // two-float KAPPA^2 sum_k |a_k|^2 of the quantised coordinates, true scale (Angstrom^2)
+    float pw;           // 2^e, e = the model's scale exponent clamped to [-30, 30]
+    float pad;
 };
 
 // ---- tensor-core engine geometry (gram_i8tc.cuh) ---------------------------------------------------

@@ -58,10 +58,12 @@ __global__ void __launch_bounds__(256) i8_plane_kernel(const float* __restrict__
     double mean[3] = {0.0, 0.0, 0.0};
     double scale = 0.0;
     int ex = 0;
+    bool finite_range = true;
     if (valid) {
         const ModelStat s = stats[n];
         mean[0] = s.mean[0]; mean[1] = s.mean[1]; mean[2] = s.mean[2];
-        ex = s.ex;
+        ex = max(-30, min(30, s.ex));
+        finite_range = s.ex <= 30;                         // coordinates beyond 2^30 Angstrom are not representable
         scale = ldexp(I8_KAPPA, 23 - ex);
     }
     const float* x = coords + n * (int64_t)L * 3;
@@ -113,13 +115,13 @@ __global__ void __launch_bounds__(256) i8_plane_kernel(const float* __restrict__
     for (int o = 16; o > 0; o >>= 1) sumsq += __shfl_xor_sync(0xffffffffu, sumsq, o);
     finite = __all_sync(0xffffffffu, finite);
     if (lane == 0) {
-        const double S = (double)sumsq * 0x1p-46;          // units: (KAPPA 2^-ex)^2 Angstrom^2
+        const double T = ldexp((double)sumsq, 2 * ex - 46);          // KAPPA^2 sum |a|^2, Angstrom^2
         PairStat ps;
-        ps.Shi = (float)S;
-        ps.Slo = (float)(S - (double)ps.Shi);
-        if (!finite) ps.Shi = __int_as_float(0x7fc00000);  // NaN/Inf coordinates poison this model's pairs
-        ps.ex = ex;
-        ps.pad = 0;
+        ps.Thi = (float)T;
+        ps.Tlo = (float)(T - (double)ps.Thi);
+        if (!finite || !finite_range) ps.Thi = __int_as_float(0x7fc00000);  // NaN/Inf coordinates poison this model's pairs
+        ps.pw = pow2i(ex);
+        ps.pad = 0.0f;
         pstat[n] = ps;
     }
 }
@@ -360,7 +362,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                     const int64_t j = J * I8_COL_MODELS + half * 8 + 4 * e + c4;
                     if (j < P.N && j > i) {
                         const PairStat sj = P.pstat[j];
-                        P.out[rowoff + j] = eq2_crmsd(m[e], si.Shi, si.Slo, si.ex, sj.Shi, sj.Slo, sj.ex, P.invLk);
+                        P.out[rowoff + j] = eq2_finish(eq2_energy(m[e]), si.Thi, si.Tlo, si.pw, sj.Thi, sj.Tlo, sj.pw, P.invLk);
                     }
                 }
             }
