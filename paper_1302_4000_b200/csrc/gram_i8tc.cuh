@@ -35,7 +35,8 @@ constexpr int I8_KC = 4;                      // k-steps per B stage: one barrie
 constexpr int I8_STAGE_BYTES = I8_KC * I8_B_SLAB;
 constexpr int I8_MAX_STAGES = 8;               // B stages in flight: as many as shared memory holds, up to this
 constexpr int I8_ACC_COLS = 144;               // TMEM columns per accumulator buffer (3 levels x 48)
-constexpr int I8_ACC_BUFS = 3;
+constexpr int I8_ACC_BUFS = 2;
+constexpr int I8_A_TMEM_COL = I8_ACC_BUFS * I8_ACC_COLS;   // the A tile lives in TMEM columns 288 .. 288 + 24 ksteps
 constexpr int I8_EPI_WARPS = 16;
 constexpr int I8_THREADS = (2 + I8_EPI_WARPS) * 32;
 
@@ -244,10 +245,20 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         constexpr uint64_t DESC_HI = (uint64_t)((256u >> 4) | (1u << 14)) << 32;
         const uint32_t a_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sA) & 0x3FFFFu) >> 4);
         const uint32_t b_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sB) & 0x3FFFFu) >> 4);
-        const uint32_t a_digit = (uint32_t)ks * (I8_A_SLAB >> 4);
+        const uint32_t a_digit = 8u * ks;                    // TMEM columns per digit
+        const uint32_t a_tm0 = tmem + I8_A_TMEM_COL;
         for (int64_t t = t0; t < t1; ++t, ++n) {
             if (I != curI) {
+                // new row tile: move its A operand from the shared-memory staging area into tensor memory
+                // (tcgen05.cp runs in order with the MMAs, so the previous row's MMAs are done reading)
                 ptx::mbar_wait(A_FULL, a_uses & 1);
+                ptx::tc_fence_after();
+                if (ptx::elect_one()) {
+                    for (int s = 0; s < 3 * ks; ++s)
+                        ptx::tmem_cp_128x256b(a_tm0 + 8 * s, DESC_HI | (a_lo0 + s * (I8_A_SLAB >> 4)));
+                    ptx::tc_commit(A_EMPTY);
+                }
+                __syncwarp();
                 ++a_uses;
                 curI = I;
             }
@@ -258,16 +269,16 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 ptx::mbar_wait(B_FULL(stage), phase);
                 ptx::tc_fence_after();
                 if (ptx::elect_one()) {
-                    const uint32_t a_lo = a_lo0 + k0 * (I8_A_SLAB >> 4);
+                    const uint32_t a_tm = a_tm0 + 8 * k0;
                     const uint32_t b_lo = b_lo0 + stage * (I8_STAGE_BYTES >> 4);
 #pragma unroll
                     for (int k = 0; k < I8_KC; ++k) {
                         if (k0 + k < ks) {
                             const uint64_t db = DESC_HI | (b_lo + k * (I8_B_SLAB >> 4));
-                            const uint32_t ak = a_lo + k * (I8_A_SLAB >> 4);
-                            ptx::mma_i8(d, DESC_HI | ak, db, ID144, (k0 + k) > 0);
-                            ptx::mma_i8(d + 48, DESC_HI | (ak + a_digit), db, ID96, 1);
-                            ptx::mma_i8(d + 96, DESC_HI | (ak + 2 * a_digit), db, ID48, 1);
+                            const uint32_t ak = a_tm + 8 * k;
+                            ptx::mma_i8_ts(d, ak, db, ID144, (k0 + k) > 0);
+                            ptx::mma_i8_ts(d + 48, ak + a_digit, db, ID96, 1);
+                            ptx::mma_i8_ts(d + 96, ak + 2 * a_digit, db, ID48, 1);
                         }
                     }
                     ptx::tc_commit(B_EMPTY(stage));
@@ -276,10 +287,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
             }
             if (++J >= Tc) { ++I; J = 2 * I; }
-            if (ptx::elect_one()) {
-                ptx::tc_commit(ACC_FULL(buf));
-                if (I != curI || t + 1 == t1) ptx::tc_commit(A_EMPTY);
-            }
+            if (ptx::elect_one()) ptx::tc_commit(ACC_FULL(buf));
             __syncwarp();
         }
     } else {
