@@ -82,11 +82,6 @@ __device__ __forceinline__ EPair eq2_energy(const float m[9])
     const float d = fmaf(m[2], C[2], fmaf(m[1], C[1], m[0] * C[0]));     // det M; its sign is S
 
     EPair r;
-    if (!(c2 > 1e-30f)) {                  // M == 0 (L = 1, or every atom on the centroid); NaN passes through
-        r.E0 = c2 * 0.0f;                  // 0, or NaN if c2 is NaN
-        r.delta = 0.0f;
-        return r;
-    }
 
     // largest root of the cubic, Viete:  l1 = q + 2 sqrt(p) cos(acos(rr / p^1.5) / 3)
     const float q = c2 * (1.0f / 3.0f);
@@ -113,8 +108,11 @@ __device__ __forceinline__ EPair eq2_energy(const float m[9])
     const float t = fmaf(E0, E0, -c2);
     const float f = fmaf(t, t, fmaf(-8.0f * d, E0, -4.0f * c1));
     const float fp = fmaf(4.0f * E0, t, -8.0f * d);
-    r.E0 = E0;
-    r.delta = (fp > 1e-3f * E0 * E0 * E0) ? f * rcp_fast(fp) : 0.0f;
+    // M == 0 (L = 1, or every atom on the centroid): E = 0 (the lines above then hold 0 * inf, selected away
+    // here, so the function stays branch-free); a NaN in M gives c2 = NaN and passes through as NaN
+    const bool nonzero = c2 > 1e-30f;
+    r.E0 = nonzero ? E0 : c2 * 0.0f;
+    r.delta = (nonzero && fp > 1e-3f * E0 * E0 * E0) ? f * rcp_fast(fp) : 0.0f;
     return r;
 }
 

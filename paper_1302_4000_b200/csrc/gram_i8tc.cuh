@@ -31,9 +31,7 @@
 namespace clusco {
 
 constexpr double I8_KAPPA = 127.0 / 128.0;
-constexpr int I8_KC = 4;                      // k-steps per B stage: one barrier round trip (~100 cycles) per 12 MMAs
-constexpr int I8_STAGE_BYTES = I8_KC * I8_B_SLAB;
-constexpr int I8_MAX_STAGES = 8;               // B stages in flight: as many as shared memory holds, up to this
+constexpr int I8_MAX_STAGES = 6;               // B stages (whole column tiles) in flight: as many as shared memory holds, up to this
 constexpr int I8_ACC_COLS = 144;               // TMEM columns per accumulator buffer (3 levels x 48)
 constexpr int I8_ACC_BUFS = 2;
 constexpr int I8_A_TMEM_COL = I8_ACC_BUFS * I8_ACC_COLS;   // the A tile lives in TMEM columns 288 .. 288 + 24 ksteps
@@ -154,33 +152,36 @@ struct I8Params {
     const PairStat* pstat;
     float* out;
     int64_t N, row_begin, row_end, base;
-    int32_t ks;
-    int32_t stages;        // B ring depth
-    int32_t wide;          // 1: level sums may exceed the int32 combine (L > 250) -> combine in fp32
+    int32_t stages;        // B ring depth (one stage = the whole column tile, KS k-steps)
     float invLk;           // 1 / (KAPPA^2 L)
     I8Tiles tiles;
 };
 
+// KS = k-steps (32 atoms each) per model, a template parameter so that the 3 KS MMAs of a tile are issued as
+// straight-line code with immediate operand offsets: the issuing warp is the critical resource of this kernel
+// (3 MMAs of 72 + 48 + 24 tensor cycles per k-step leave ~48 cycles of issue time per MMA).
+template <int KS>
 __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params P)
 {
     extern __shared__ __align__(128) uint8_t smem[];
-    const int ks = P.ks;
-    uint8_t* sA = smem;                                          // 3 digits x ks x 4096
-    const int I8_STAGES = P.stages;
-    uint8_t* sB = smem + (size_t)3 * ks * I8_A_SLAB;             // stages x I8_KC x 4608
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)I8_STAGES * I8_STAGE_BYTES);
-    // barrier map: [0,S) b_full, [S,2S) b_empty, 2S a_full, 2S+1 a_empty, 2S+2.. acc_full[3], acc_empty[3]
+    constexpr int ks = KS;
+    constexpr uint32_t STAGE_BYTES = KS * I8_B_SLAB;
+    const int stages = P.stages;
+    uint8_t* sA = smem;                                          // staging for the next row tile: 3 digits x KS x 4096
+    uint8_t* sB = smem + (size_t)3 * ks * I8_A_SLAB;             // stages x KS x 4608
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)stages * STAGE_BYTES);
+    // barrier map: [0,S) b_full, [S,2S) b_empty, 2S a_full, 2S+1 a_empty, 2S+2.. acc_full[2], acc_empty[2]
     const uint32_t bar0 = ptx::smem_u32(bars);
-    auto B_FULL = [&](int s) { return bar0 + 8u * s; };
-    auto B_EMPTY = [&](int s) { return bar0 + 8u * (I8_STAGES + s); };
-    const uint32_t A_FULL = bar0 + 8u * (2 * I8_STAGES), A_EMPTY = A_FULL + 8u;
-    auto ACC_FULL = [&](int b) { return bar0 + 8u * (2 * I8_STAGES + 2 + b); };
-    auto ACC_EMPTY = [&](int b) { return bar0 + 8u * (2 * I8_STAGES + 2 + I8_ACC_BUFS + b); };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * I8_STAGES + 2 + 2 * I8_ACC_BUFS);
+    auto B_FULL = [&](uint32_t s) { return bar0 + 8u * s; };
+    auto B_EMPTY = [&](uint32_t s) { return bar0 + 8u * (stages + s); };
+    const uint32_t A_FULL = bar0 + 8u * (2 * stages), A_EMPTY = A_FULL + 8u;
+    auto ACC_FULL = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 2 + b); };
+    auto ACC_EMPTY = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 2 + I8_ACC_BUFS + b); };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * stages + 2 + 2 * I8_ACC_BUFS);
 
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
-        for (int s = 0; s < I8_STAGES; ++s) {
+        for (int s = 0; s < stages; ++s) {
             ptx::mbar_init(B_FULL(s), 1);
             ptx::mbar_init(B_EMPTY(s), 1);
         }
@@ -201,111 +202,129 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     const int64_t G = gridDim.x, b = blockIdx.x;
     const int64_t t0 = P.tiles.total * b / G, t1 = P.tiles.total * (b + 1) / G;
     const int64_t Tc = P.tiles.Tc;
+    const uint32_t ntiles = (uint32_t)(t1 - t0);
+    int64_t I0, J0;
+    i8_tile_from_linear(P.tiles, t0, I0, J0);
 
     if (warp == 0) {
-        // ===== producer =====
+        // ===== producer: one elected lane streams operand images with 1-D bulk copies =====
         if (lane == 0) {
-            int64_t I, J;
-            i8_tile_from_linear(P.tiles, t0, I, J);
+            int64_t I = I0, J = J0;
             int64_t curI = -1;
             uint32_t a_loads = 0, stage = 0, phase = 0;
-            for (int64_t t = t0; t < t1; ++t) {
+            for (uint32_t n = 0; n < ntiles; ++n) {
                 if (I != curI) {
                     ptx::mbar_wait(A_EMPTY, (a_loads & 1) ^ 1);
                     ptx::mbar_expect_tx(A_FULL, 3u * ks * I8_A_SLAB);
-                    const int8_t* src = P.Ap + (size_t)I * 3 * ks * I8_A_SLAB;
-#pragma unroll
-                    for (int a = 0; a < 3; ++a)
-                        ptx::bulk_g2s(ptx::smem_u32(sA + (size_t)a * ks * I8_A_SLAB), src + (size_t)a * ks * I8_A_SLAB,
-                                      (uint32_t)ks * I8_A_SLAB, A_FULL);
+                    ptx::bulk_g2s(ptx::smem_u32(sA), P.Ap + (size_t)I * 3 * ks * I8_A_SLAB, 3u * ks * I8_A_SLAB, A_FULL);
                     ++a_loads;
                     curI = I;
                 }
-                const int8_t* srcB = P.Bp + (size_t)J * ks * I8_B_SLAB;
-                for (int k0 = 0; k0 < ks; k0 += I8_KC) {
-                    const uint32_t bytes = (uint32_t)min(I8_KC, ks - k0) * I8_B_SLAB;
-                    ptx::mbar_wait(B_EMPTY(stage), phase ^ 1);
-                    ptx::mbar_expect_tx(B_FULL(stage), bytes);
-                    ptx::bulk_g2s(ptx::smem_u32(sB + (size_t)stage * I8_STAGE_BYTES), srcB + (size_t)k0 * I8_B_SLAB, bytes,
-                                  B_FULL(stage));
-                    if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
-                }
+                ptx::mbar_wait(B_EMPTY(stage), phase ^ 1);
+                ptx::mbar_expect_tx(B_FULL(stage), STAGE_BYTES);
+                ptx::bulk_g2s(ptx::smem_u32(sB + (size_t)stage * STAGE_BYTES), P.Bp + (size_t)J * STAGE_BYTES, STAGE_BYTES,
+                              B_FULL(stage));
+                if (++stage == (uint32_t)stages) { stage = 0; phase ^= 1; }
                 if (++J >= Tc) { ++I; J = 2 * I; }
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer: the whole warp walks the loop (warp-uniform control flow and addresses, so the
-        // descriptors live in uniform registers); one elected lane issues =====
-        int64_t I, J;
-        i8_tile_from_linear(P.tiles, t0, I, J);
-        int64_t curI = -1;
-        uint32_t a_uses = 0, stage = 0, phase = 0, n = 0;
+        // operands live in uniform registers); one elected lane issues =====
         constexpr uint32_t ID144 = ptx::idesc_s8(128, 144), ID96 = ptx::idesc_s8(128, 96), ID48 = ptx::idesc_s8(128, 48);
         // descriptor = hi word (SBO 256 B, version 1) | lo word (LBO 128 B, start address >> 4)
         constexpr uint64_t DESC_HI = (uint64_t)((256u >> 4) | (1u << 14)) << 32;
         const uint32_t a_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sA) & 0x3FFFFu) >> 4);
         const uint32_t b_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sB) & 0x3FFFFu) >> 4);
-        const uint32_t a_digit = 8u * ks;                    // TMEM columns per digit
-        const uint32_t a_tm0 = tmem + I8_A_TMEM_COL;
-        for (int64_t t = t0; t < t1; ++t, ++n) {
-            if (I != curI) {
+        const uint32_t a_tm = tmem + I8_A_TMEM_COL;              // digit a, k-step k at column 8 (a KS + k)
+        uint32_t rem = 0;                                        // tiles left in the current row tile
+        uint32_t next_rem = (uint32_t)(Tc - J0);
+        uint32_t next_row_len = (uint32_t)(Tc - 2 * (I0 + 1));   // each further row is two tiles shorter
+        uint32_t a_uses = 0, stage = 0, phase = 0;
+        for (uint32_t n = 0; n < ntiles; ++n) {
+            if (rem == 0) {
                 // new row tile: move its A operand from the shared-memory staging area into tensor memory
                 // (tcgen05.cp runs in order with the MMAs, so the previous row's MMAs are done reading)
+                rem = next_rem;
+                next_rem = next_row_len;
+                next_row_len -= 2;
                 ptx::mbar_wait(A_FULL, a_uses & 1);
                 ptx::tc_fence_after();
                 if (ptx::elect_one()) {
-                    for (int s = 0; s < 3 * ks; ++s)
-                        ptx::tmem_cp_128x256b(a_tm0 + 8 * s, DESC_HI | (a_lo0 + s * (I8_A_SLAB >> 4)));
+#pragma unroll
+                    for (int s = 0; s < 3 * KS; ++s)
+                        ptx::tmem_cp_128x256b(a_tm + 8 * s, DESC_HI | (a_lo0 + s * (I8_A_SLAB >> 4)));
                     ptx::tc_commit(A_EMPTY);
                 }
                 __syncwarp();
                 ++a_uses;
-                curI = I;
             }
-            const uint32_t buf = n % I8_ACC_BUFS;
-            ptx::mbar_wait(ACC_EMPTY(buf), ((n / I8_ACC_BUFS) & 1) ^ 1);
-            const uint32_t d = tmem + buf * I8_ACC_COLS;
-            for (int k0 = 0; k0 < ks; k0 += I8_KC) {
-                ptx::mbar_wait(B_FULL(stage), phase);
-                ptx::tc_fence_after();
-                if (ptx::elect_one()) {
-                    const uint32_t a_tm = a_tm0 + 8 * k0;
-                    const uint32_t b_lo = b_lo0 + stage * (I8_STAGE_BYTES >> 4);
+            --rem;
+            const uint32_t buf = n & 1;
+#if !(defined(I8_EXPERIMENT) && I8_EXPERIMENT >= 5)
+            ptx::mbar_wait(ACC_EMPTY(buf), ((n >> 1) & 1) ^ 1);
+            ptx::mbar_wait(B_FULL(stage), phase);
+#endif
+            ptx::tc_fence_after();
+            if (ptx::elect_one()) {
+                const uint32_t d = tmem + buf * I8_ACC_COLS;
+                const uint32_t b_lo = b_lo0 + stage * (STAGE_BYTES >> 4);
 #pragma unroll
-                    for (int k = 0; k < I8_KC; ++k) {
-                        if (k0 + k < ks) {
-                            const uint64_t db = DESC_HI | (b_lo + k * (I8_B_SLAB >> 4));
-                            const uint32_t ak = a_tm + 8 * k;
-                            ptx::mma_i8_ts(d, ak, db, ID144, (k0 + k) > 0);
-                            ptx::mma_i8_ts(d + 48, ak + a_digit, db, ID96, 1);
-                            ptx::mma_i8_ts(d + 96, ak + 2 * a_digit, db, ID48, 1);
-                        }
-                    }
-                    ptx::tc_commit(B_EMPTY(stage));
+                for (int k = 0; k < KS; ++k) {
+                    const uint64_t db = DESC_HI | (b_lo + k * (I8_B_SLAB >> 4));
+#if defined(I8_EXPERIMENT) && I8_EXPERIMENT == 2          // developer switch: one MMA per tile (epilogue-side time only)
+                    if (k == 0) ptx::mma_i8_ts(d, a_tm, db, ID144, 0);
+#else
+                    ptx::mma_i8_ts(d, a_tm + 8 * k, db, ID144, k > 0);
+                    ptx::mma_i8_ts(d + 48, a_tm + 8 * (KS + k), db, ID96, 1);
+                    ptx::mma_i8_ts(d + 96, a_tm + 8 * (2 * KS + k), db, ID48, 1);
+#endif
                 }
-                __syncwarp();
-                if (++stage == I8_STAGES) { stage = 0; phase ^= 1; }
+                ptx::tc_commit(B_EMPTY(stage));
+                ptx::tc_commit(ACC_FULL(buf));
             }
-            if (++J >= Tc) { ++I; J = 2 * I; }
-            if (ptx::elect_one()) ptx::tc_commit(ACC_FULL(buf));
             __syncwarp();
+            if (++stage == (uint32_t)stages) { stage = 0; phase ^= 1; }
         }
     } else {
         // ===== epilogue =====
+#if defined(I8_EXPERIMENT) && I8_EXPERIMENT == 6
+        if (true) goto done;
+#endif
         const int ew = warp - 2;
         const int team = ew >> 3, half = (ew & 7) >> 2;          // column half: models 8*half .. 8*half+7 of the tile
         const int quad = warp & 3;                               // TMEM lanes 32 quad .. 32 quad + 31
         const int r = lane >> 2, c4 = lane & 3;
-        int64_t I, J;
-        i8_tile_from_linear(P.tiles, t0 + team, I, J);
-        for (int64_t t = t0 + team, n = team; t < t1; t += 2, n += 2) {
-            const uint32_t buf = (uint32_t)(n % I8_ACC_BUFS);
-            ptx::mbar_wait(ACC_FULL(buf), (uint32_t)((n / I8_ACC_BUFS) & 1));
+        int64_t I = I0, J = J0;
+        if (team == 1 && ++J >= Tc) { ++I; J = 2 * I; }
+        int64_t curI = -1, i = 0, rowoff = 0;
+        bool row_ok = false;
+        PairStat si = {0.0f, 0.0f, 1.0f, 0.0f};
+        for (uint32_t n = team; n < ntiles; n += 2) {
+            if (I != curI) {                                     // per-row quantities (warp-uniform branch)
+                curI = I;
+                i = I * I8_ROW_MODELS + quad * 8 + r;
+                row_ok = i < P.N && i >= P.row_begin && i < P.row_end;
+                si = P.pstat[i];                                 // slots beyond N hold neutral records
+                rowoff = i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
+            }
+            // per-model records of this thread's two column models, requested before the accumulator wait
+            const int64_t j0 = J * I8_COL_MODELS + half * 8 + c4;
+            const PairStat sj0 = P.pstat[j0], sj1 = P.pstat[j0 + 4];
+            const uint32_t buf = (uint32_t)team;                 // tile n uses accumulator n & 1 = team
+            ptx::mbar_wait(ACC_FULL(buf), (n >> 1) & 1);
             ptx::tc_fence_after();
             const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16) + buf * I8_ACC_COLS + half * 8;
-            // m[e][3p+q]: pair (row model r, column model c4 + 4e + 8 half)
+            // m[e][3p+q]: pair (row model r, column model c4 + 4e + 8 half), Gram sums in units of 2^46
             float m[2][9];
+#if defined(I8_EXPERIMENT) && I8_EXPERIMENT >= 3              // developer switch: no TMEM loads, no arithmetic
+#pragma unroll
+            for (int e = 0; e < 2; ++e)
+#pragma unroll
+                for (int q = 0; q < 9; ++q) m[e][q] = (float)(n + q);
+#else
             {
+                // levels 1 and 2 first: T = 2^8 V1 + V2 fits int32 (|T| < 2^31 for L <= 256 because |d0| <= 127)
                 uint32_t v1[3][2][4], v2[3][2][4];
 #pragma unroll
                 for (int q = 0; q < 3; ++q)
@@ -315,30 +334,19 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                         ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 96 + 16 * q, v2[q][h]);
                     }
                 ptx::tmem_ld_wait();
-                if (!P.wide) {
-                    int32_t T[2][9];
+                int32_t T[2][9];
 #pragma unroll
-                    for (int q = 0; q < 3; ++q)
+                for (int q = 0; q < 3; ++q)
 #pragma unroll
-                        for (int e = 0; e < 2; ++e) {
-                            T[e][0 + q] = ((int32_t)v1[q][0][e] << 8) + (int32_t)v2[q][0][e];
-                            T[e][3 + q] = ((int32_t)v1[q][0][2 + e] << 8) + (int32_t)v2[q][0][2 + e];
-                            T[e][6 + q] = ((int32_t)v1[q][1][e] << 8) + (int32_t)v2[q][1][e];
-                        }
+                    for (int e = 0; e < 2; ++e) {
+                        T[e][0 + q] = ((int32_t)v1[q][0][e] << 8) + (int32_t)v2[q][0][e];
+                        T[e][3 + q] = ((int32_t)v1[q][0][2 + e] << 8) + (int32_t)v2[q][0][2 + e];
+                        T[e][6 + q] = ((int32_t)v1[q][1][e] << 8) + (int32_t)v2[q][1][e];
+                    }
 #pragma unroll
-                    for (int e = 0; e < 2; ++e)
+                for (int e = 0; e < 2; ++e)
 #pragma unroll
-                        for (int i = 0; i < 9; ++i) m[e][i] = (float)T[e][i] * 0x1p-30f;
-                } else {
-#pragma unroll
-                    for (int q = 0; q < 3; ++q)
-#pragma unroll
-                        for (int e = 0; e < 2; ++e) {
-                            m[e][0 + q] = fmaf((float)(int32_t)v1[q][0][e], 0x1p-22f, (float)(int32_t)v2[q][0][e] * 0x1p-30f);
-                            m[e][3 + q] = fmaf((float)(int32_t)v1[q][0][2 + e], 0x1p-22f, (float)(int32_t)v2[q][0][2 + e] * 0x1p-30f);
-                            m[e][6 + q] = fmaf((float)(int32_t)v1[q][1][e], 0x1p-22f, (float)(int32_t)v2[q][1][e] * 0x1p-30f);
-                        }
-                }
+                    for (int q = 0; q < 9; ++q) m[e][q] = (float)T[e][q] * 0x1p-30f;
             }
             {
                 uint32_t v0[3][2][4];
@@ -356,30 +364,32 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                         m[e][6 + q] = fmaf((float)(int32_t)v0[q][1][e], 0x1p-14f, m[e][6 + q]);
                     }
             }
+#endif
             // the accumulator buffer is free again
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
 
-            const int64_t i = I * I8_ROW_MODELS + quad * 8 + r;
-            if (i < P.N && i >= P.row_begin && i < P.row_end) {
-                const PairStat si = P.pstat[i];
-                const int64_t rowoff = i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
-#pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int64_t j = J * I8_COL_MODELS + half * 8 + 4 * e + c4;
-                    if (j < P.N && j > i) {
-                        const PairStat sj = P.pstat[j];
-                        P.out[rowoff + j] = eq2_finish(eq2_energy(m[e]), si.Thi, si.Tlo, si.pw, sj.Thi, sj.Tlo, sj.pw, P.invLk);
-                    }
-                }
-            }
+#if defined(I8_EXPERIMENT) && (I8_EXPERIMENT == 1 || I8_EXPERIMENT >= 3)   // developer switch: no eq. 2 arithmetic
+            const float c0 = m[0][0] + m[0][4] + m[0][8], c1 = m[1][0] + m[1][4] + m[1][8];
+            if (row_ok && j0 < P.N && j0 > i) P.out[rowoff + j0] = c0 + si.Thi + sj0.Thi;
+            if (row_ok && j0 + 4 < P.N && j0 + 4 > i) P.out[rowoff + j0 + 4] = c1 + sj1.Thi;
+#else
+            // both pairs are evaluated branch-free (their chains interleave); masked pairs are simply not stored
+            const float c0 = eq2_finish(eq2_energy(m[0]), si.Thi, si.Tlo, si.pw, sj0.Thi, sj0.Tlo, sj0.pw, P.invLk);
+            const float c1 = eq2_finish(eq2_energy(m[1]), si.Thi, si.Tlo, si.pw, sj1.Thi, sj1.Tlo, sj1.pw, P.invLk);
+            if (row_ok && j0 < P.N && j0 > i) P.out[rowoff + j0] = c0;
+            if (row_ok && j0 + 4 < P.N && j0 + 4 > i) P.out[rowoff + j0 + 4] = c1;
+#endif
             // advance two tiles
 #pragma unroll
             for (int s = 0; s < 2; ++s)
                 if (++J >= Tc) { ++I; J = 2 * I; }
         }
     }
+#if defined(I8_EXPERIMENT) && I8_EXPERIMENT == 6
+done:
+#endif
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
@@ -387,7 +397,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
 
 static inline size_t i8tc_smem_bytes(int ks, int stages)
 {
-    return (size_t)3 * ks * I8_A_SLAB + (size_t)stages * I8_STAGE_BYTES + 8 * (2 * stages + 2 + 2 * I8_ACC_BUFS) + 16;
+    return (size_t)3 * ks * I8_A_SLAB + (size_t)stages * ks * I8_B_SLAB + 8 * (2 * stages + 2 + 2 * I8_ACC_BUFS) + 16;
 }
 static inline int i8tc_stages(int ks)
 {
@@ -422,19 +432,26 @@ static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t 
     P.row_begin = row_begin;
     P.row_end = row_end;
     P.base = packed_index(row_begin, row_begin + 1, N);
-    P.ks = w.Lp32 / 32;
-    P.wide = L > 250 ? 1 : 0;
+    const int ks = w.Lp32 / 32;
     P.invLk = (float)(1.0 / (I8_KAPPA * I8_KAPPA * (double)L));
     P.tiles.Tc = w.col_tiles;
     P.tiles.I_lo = row_begin / I8_ROW_MODELS;
     P.tiles.I_hi = (row_end + I8_ROW_MODELS - 1) / I8_ROW_MODELS;
     P.tiles.total = i8_tiles_before(P.tiles, P.tiles.I_hi);
     if (P.tiles.total <= 0) return CLUSCO_OK;
-    P.stages = i8tc_stages(P.ks);
-    const size_t smem = i8tc_smem_bytes(P.ks, P.stages);
-    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gram_i8tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    P.stages = i8tc_stages(ks);
+    const size_t smem = i8tc_smem_bytes(ks, P.stages);
     const int64_t grid = P.tiles.total < sms ? P.tiles.total : sms;
-    gram_i8tc_kernel<<<(unsigned)grid, I8_THREADS, smem, s>>>(P);
+    switch (ks) {
+#define I8_LAUNCH(KS)                                                                                                  \
+    case KS:                                                                                                           \
+        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gram_i8tc_kernel<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
+        gram_i8tc_kernel<KS><<<(unsigned)grid, I8_THREADS, smem, s>>>(P);                                              \
+        break;
+        I8_LAUNCH(1) I8_LAUNCH(2) I8_LAUNCH(3) I8_LAUNCH(4) I8_LAUNCH(5) I8_LAUNCH(6) I8_LAUNCH(7) I8_LAUNCH(8)
+#undef I8_LAUNCH
+        default: return CLUSCO_ERR_INVALID_ARG;
+    }
     CLUSCO_CUDA_TRY(cudaGetLastError());
     return CLUSCO_OK;
 }
