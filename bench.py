@@ -142,6 +142,7 @@ def main():
     ap.add_argument("--engine", default="auto", choices=["auto", "ffma", "i8tc"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-ova", action="store_true", help="skip the one-vs-all (C5) side measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -242,22 +243,39 @@ def main():
             dist.destroy_process_group()
         return
 
-    # roofline for the dominant kernel (the fused Gram+epilogue kernel): algorithmic flops 18*L per pair
+    # roofline for the dominant kernel (the fused Gram + eq. 2 + store kernel): ALGORITHMIC flops = 18 L per pair
+    # (9 L multiply-adds; upper triangle only -- padding rows, diagonal-tile waste and the six digit products of
+    # the exact int8 split are NOT counted), DESIGN.md section 7
     pk = _peaks()
     flops = 18.0 * L * P
+    achieved = flops / (kern_ms * 1e-3) / 1e12
     if engine == clusco.ENGINE_FFMA:
         peak = 148 * 128 * 2 * pk["sm_max_mhz"] * 1e6 / 1e12          # FP32 FFMA: #SM x 128 lanes x 2 x clock
-        roof = {"bound": "alu", "achieved": flops / (kern_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
-                "peak_source": "148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz (DESIGN.md)"}
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "peak_source": "148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz (DESIGN.md 7.1)"}
     else:
-        peak = 2.0 * pk["bf16_tflops"]                                # int8 dense = 2x bf16 (nominal ratio)
-        roof = {"bound": "tensor", "achieved": flops / (kern_ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
-                "peak_source": f"2 x {pk['source']} bf16 burst peak (int8:bf16 nominal ratio)"}
+        peak = 2.0 * pk["bf16_tflops"]                                # int8 dense = 2x bf16 (the guide's nominal ratio)
+        # what the tensor pipe actually executes: tiles x k-steps x (144+96+48) columns x 128 rows x 32 atoms
+        Tc, Tr, ks = (N + 15) // 16, (N + 31) // 32, (L + 31) // 32
+        tiles = sum(Tc - 2 * i for i in range(Tr))
+        issued = 2.0 * tiles * ks * 288 * 128 * 32
+        roof = {"bound": "tensor", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                "peak_source": f"int8 tensor peak = 2 x {pk['source']} bf16 burst ({pk['bf16_tflops']:.0f} TFLOP/s), "
+                               "nominal int8:bf16 ratio (of measured)",
+                "issued_tops": issued / (kern_ms * 1e-3) / 1e12,
+                "issued_frac": issued / (kern_ms * 1e-3) / 1e12 / peak,
+                "issued_over_algorithmic": issued / flops}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
     roof["kernel_ms"] = kern_ms
     roof["kernel"] = "gram_ffma_kernel" if engine == clusco.ENGINE_FFMA else "gram_i8tc_kernel"
+    roof["kernel_share_of_step"] = kern_ms / ms_per_step
+    roof["traffic"] = _ncu_traffic(roof["kernel"], args.workload)
+    roof["algorithmic_bytes"] = 4.0 * P + 12.0 * N * L
     roof["hbm_bound_ms"] = (4.0 * P + 12.0 * N * L) / (pk["hbm_gbs"] * 1e9) * 1e3
+
+    ova = None
+    if not args.no_ova and world == 1:
+        ova = one_vs_all_side(clusco, wl, pk, flush)
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -266,17 +284,62 @@ def main():
     print(json.dumps({
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32" if engine == clusco.ENGINE_FFMA else "s8 x s8 -> s32 (3x8-bit fixed point), f32 epilogue",
+        "vs_baseline": None, "dtype": "f32" if engine == clusco.ENGINE_FFMA else "s8",
         "data": "synthetic",
         "config": {"workload": f"{args.workload}: N={N} models x L={L} C-alpha, all-vs-all packed upper triangle "
                                f"({P} pairs), one ensemble per GPU",
                    "engine": {1: "ffma", 2: "i8tc"}[engine], "l2": "flushed between timed iterations (256 MB write)",
                    "effective_tflops": flops * world / (ms_per_step * 1e-3) / 1e12},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step(engine) * args.steps,
-        "roofline": roof, "cpu_baseline": cpu,
+        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova,
     }))
     if dist:
         dist.destroy_process_group()
+
+
+def _ncu_traffic(kernel, workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` capture."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    best = None
+    for line in open(path):
+        f = [c.strip() for c in line.split(",")]
+        if len(f) >= 4 and f[0] == kernel and f[1] == workload:
+            best = float(f[2]) + float(f[3])          # last matching row = latest round
+    return best
+
+
+def one_vs_all_side(clusco, wl, pk, flush):
+    """Step a6 on its own workload (C5: one native vs 10^6 models x 150 atoms, 1.8 GB): HBM-bound single pass."""
+    import torch
+    N, L, chunk = 1_000_000, 150, 100_000
+    ens0 = wl.make_config("C5", N=N, chunk=chunk, chunks=range(0))
+    coords = torch.empty((N, L, 3), dtype=torch.float32, device="cuda")
+    for k in range(N // chunk):
+        part = wl.make_config("C5", N=N, chunk=chunk, chunks=range(k, k + 1))
+        coords[k * chunk:(k + 1) * chunk] = torch.from_numpy(part.coords).cuda()
+    native = torch.from_numpy(ens0.native).cuda()
+    out = torch.empty(N, dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream()
+    for _ in range(3):
+        clusco.clusco_crmsd_one_vs_all(native, coords, out)
+    reps = 10
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    torch.cuda.synchronize()
+    for a, b in ev:
+        flush.zero_()                                   # inputs (1.8 GB) exceed L2 anyway
+        a.record(stream)
+        clusco.clusco_crmsd_one_vs_all(native, coords, out)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / reps
+    nbytes = 12.0 * N * L + 4.0 * N
+    gbs = nbytes / (ms * 1e-3) / 1e9
+    return {"workload": "C5: 1 native vs N=1000000 models x L=150", "ms": ms, "models_per_s": N / (ms * 1e-3),
+            "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
+                         "frac": gbs / pk["hbm_gbs"], "traffic": _ncu_traffic("one_vs_all_kernel", "C5"),
+                         "algorithmic_bytes": nbytes, "kernel": "one_vs_all_kernel"}}
 
 
 def launches_per_step(engine):
