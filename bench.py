@@ -338,8 +338,8 @@ def one_vs_all_side(clusco, wl, pk, flush):
     gbs = nbytes / (ms * 1e-3) / 1e9
     return {"workload": "C5: 1 native vs N=1000000 models x L=150", "ms": ms, "models_per_s": N / (ms * 1e-3),
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
-                         "frac": gbs / pk["hbm_gbs"], "traffic": _ncu_traffic("one_vs_all_kernel", "C5"),
-                         "algorithmic_bytes": nbytes, "kernel": "one_vs_all_kernel"}}
+                         "frac": gbs / pk["hbm_gbs"], "traffic": _ncu_traffic("one_vs_all_stream_kernel", "C5"),
+                         "algorithmic_bytes": nbytes, "kernel": "one_vs_all_stream_kernel"}}
 
 
 def launches_per_step(engine):

@@ -202,24 +202,46 @@ int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N,
     cudaStream_t s = (cudaStream_t)stream;
     const size_t nat_bytes = (size_t)L * sizeof(float4);
     if (nat_bytes > 200 * 1024) return CLUSCO_ERR_INVALID_ARG;        // L <= 12800 atoms
+    if (!aligned16(coords)) return CLUSCO_ERR_INVALID_ARG;
+    const size_t natc_sz = (size_t)round_up((int64_t)nat_bytes, 256);
+    const size_t natq_sz = (size_t)round_up((int64_t)((L + 3) / 4) * OVA_NATQ_FLOATS * 4, 256);
     char* scratch = nullptr;
-    CLUSCO_CUDA_TRY(cudaMallocAsync((void**)&scratch, (size_t)round_up((int64_t)nat_bytes, 256) + 256, s));
+    CLUSCO_CUDA_TRY(cudaMallocAsync((void**)&scratch, natc_sz + natq_sz + 256, s));
     float4* natc = (float4*)scratch;
-    NativeStat* nstat = (NativeStat*)(scratch + round_up((int64_t)nat_bytes, 256));
-    native_prep_kernel<<<1, 256, 0, s>>>(native, L, natc, nstat);
+    float* natq = (float*)(scratch + natc_sz);
+    NativeStat* nstat = (NativeStat*)(scratch + natc_sz + natq_sz);
+    native_prep_kernel<<<1, 256, 0, s>>>(native, L, natc, natq, nstat);
     CLUSCO_CUDA_TRY(cudaGetLastError());
-    static thread_local size_t smem_set = 0;
-    if (nat_bytes > 48 * 1024 && nat_bytes > smem_set) {
-        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(one_vs_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)nat_bytes));
-        smem_set = nat_bytes;
-    }
     const int64_t n_blocks32 = (N + 31) / 32;
-    int64_t grid = (n_blocks32 + OVA_WARPS - 1) / OVA_WARPS;
-    const int64_t cap = (int64_t)sms * 8;
-    if (grid > cap) grid = cap;
-    one_vs_all_kernel<<<(unsigned)grid, OVA_WARPS * 32, nat_bytes, s>>>(natc, nstat, coords, N, L,
-                                                                       1.0f / (float)L, out);
+    int warps = 0, stages = 0;
+    if (ova_stream_config(L, &warps, &stages)) {
+        // streaming kernel: one persistent CTA per SM, every warp walks batches of 32 models
+        const size_t smem = ova_stream_smem(L, warps, stages);
+        int64_t grid = (n_blocks32 + warps - 1) / warps;
+        if (grid > sms) grid = sms;
+        const int vec = (L % 4 == 0) ? 4 : (L % 2 == 0 ? 2 : 1);
+#define OVA_LAUNCH(V)                                                                                                  \
+    do {                                                                                                               \
+        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(one_vs_all_stream_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                             (int)smem));                                                              \
+        one_vs_all_stream_kernel<V><<<(unsigned)grid, warps * 32, smem, s>>>(natq, nstat, coords, N, L,                \
+                                                                             1.0f / (float)L, stages, out);            \
+    } while (0)
+        if (vec == 4) OVA_LAUNCH(4); else if (vec == 2) OVA_LAUNCH(2); else OVA_LAUNCH(1);
+#undef OVA_LAUNCH
+    } else {
+        static thread_local size_t smem_set = 0;
+        if (nat_bytes > 48 * 1024 && nat_bytes > smem_set) {
+            CLUSCO_CUDA_TRY(cudaFuncSetAttribute(one_vs_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                 (int)nat_bytes));
+            smem_set = nat_bytes;
+        }
+        int64_t grid = (n_blocks32 + OVA_WARPS - 1) / OVA_WARPS;
+        const int64_t cap = (int64_t)sms * 8;
+        if (grid > cap) grid = cap;
+        one_vs_all_kernel<<<(unsigned)grid, OVA_WARPS * 32, nat_bytes, s>>>(natc, nstat, coords, N, L,
+                                                                           1.0f / (float)L, out);
+    }
     CLUSCO_CUDA_TRY(cudaGetLastError());
     CLUSCO_CUDA_TRY(cudaFreeAsync(scratch, s));
     return CLUSCO_OK;

@@ -190,7 +190,10 @@ def test_one_vs_all_prefix(clusco):
     print(f"C5 20000-model prefix: max|dc2| = {worst:.2e}")
 
 
-@pytest.mark.parametrize("N,L", [(1, 3), (31, 2), (33, 150), (1000, 37), (77, 887)])
+# L % 4 == 0 / even / odd select the three vector widths of the streaming kernel; N % 4 != 0 with 12 L (N % 4)
+# not a multiple of 16 takes the plain-load tail; L > 2048 takes the long-chain kernel
+@pytest.mark.parametrize("N,L", [(1, 3), (2, 1), (31, 2), (6, 4), (33, 150), (130, 152), (35, 151), (1000, 37),
+                                 (4099, 36), (77, 887), (3, 2100)])
 def test_one_vs_all_ragged(clusco, N, L):
     rng = np.random.default_rng(7 * N + L)
     nat = wl.random_walk_chain(L, rng)
