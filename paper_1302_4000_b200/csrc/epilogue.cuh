@@ -21,99 +21,160 @@
 
 namespace clusco {
 
-struct EPair { float E0; float delta; };
-
 // ---- fast single-instruction approximations (MUFU), relative error ~2^-22; every use below is either polished
 // by the Newton step that follows or far inside the output tolerance ---------------------------------------
 __device__ __forceinline__ float rcp_fast(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_fast(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float sqrt_fast(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float cos_fast(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-// acos on [-1, 1]: sqrt(1 - |x|) * P7(|x|)  (Abramowitz & Stegun 4.4.46, |error| <= 2e-8), reflected for x < 0
-__device__ __forceinline__ float acos_fast(float x)
+
+// ---- the arithmetic of the closed form, written once for V = float (one pair per thread) and V = float2 (two
+// pairs per thread, evaluated together on the packed FFMA2 / FMUL2 / FADD2 instructions of sm_100; operand
+// negation and scalar broadcast fold into those instructions).  Comparisons, selects and MUFU stay per lane. ---
+namespace lp {
+template <class V> __device__ __forceinline__ V splat(float s);
+template <> __device__ __forceinline__ float splat<float>(float s) { return s; }
+template <> __device__ __forceinline__ float2 splat<float2>(float s) { return make_float2(s, s); }
+
+__device__ __forceinline__ float fma(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ float2 fma(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float mul(float a, float b) { return a * b; }
+__device__ __forceinline__ float2 mul(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float add(float a, float b) { return a + b; }
+__device__ __forceinline__ float2 add(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float neg(float a) { return -a; }
+__device__ __forceinline__ float2 neg(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float sub(float a, float b) { return a - b; }
+__device__ __forceinline__ float2 sub(float2 a, float2 b) { return __fadd2_rn(a, neg(b)); }
+// per-lane map / zip for the operations that have no packed form
+template <class F> __device__ __forceinline__ float map(float a, F f) { return f(a); }
+template <class F> __device__ __forceinline__ float2 map(float2 a, F f) { return make_float2(f(a.x), f(a.y)); }
+template <class F> __device__ __forceinline__ float zip(float a, float b, F f) { return f(a, b); }
+template <class F> __device__ __forceinline__ float2 zip(float2 a, float2 b, F f) { return make_float2(f(a.x, b.x), f(a.y, b.y)); }
+template <class F> __device__ __forceinline__ float zip3(float a, float b, float c, F f) { return f(a, b, c); }
+template <class F> __device__ __forceinline__ float2 zip3(float2 a, float2 b, float2 c, F f)
 {
-    const float ax = fabsf(x);
-    float p = -0.0012624911f;
-    p = fmaf(p, ax, 0.0066700901f);
-    p = fmaf(p, ax, -0.0170881256f);
-    p = fmaf(p, ax, 0.0308918810f);
-    p = fmaf(p, ax, -0.0501743046f);
-    p = fmaf(p, ax, 0.0889789874f);
-    p = fmaf(p, ax, -0.2145988016f);
-    p = fmaf(p, ax, 1.5707963050f);
-    const float r = sqrt_fast(1.0f - ax) * p;
-    return x < 0.0f ? 3.14159265358979f - r : r;
+    return make_float2(f(a.x, b.x, c.x), f(a.y, b.y, c.y));
+}
+}  // namespace lp
+
+template <class V> struct EPairT { V E0; V delta; };
+typedef EPairT<float> EPair;
+
+// acos on [-1, 1]: sqrt(1 - |x|) * P7(|x|)  (Abramowitz & Stegun 4.4.46, |error| <= 2e-8), reflected for x < 0
+template <class V>
+__device__ __forceinline__ V acos_fast(V x)
+{
+    using namespace lp;
+    const V ax = map(x, [](float t) { return fabsf(t); });
+    V p = splat<V>(-0.0012624911f);
+    p = fma(p, ax, splat<V>(0.0066700901f));
+    p = fma(p, ax, splat<V>(-0.0170881256f));
+    p = fma(p, ax, splat<V>(0.0308918810f));
+    p = fma(p, ax, splat<V>(-0.0501743046f));
+    p = fma(p, ax, splat<V>(0.0889789874f));
+    p = fma(p, ax, splat<V>(-0.2145988016f));
+    p = fma(p, ax, splat<V>(1.5707963050f));
+    const V r = mul(map(sub(splat<V>(1.0f), ax), [](float t) { return sqrt_fast(t); }), p);
+    return zip(x, r, [](float xx, float rr) { return xx < 0.0f ? 3.14159265358979f - rr : rr; });
 }
 
 // a*b - c*d with one rounding error of the result (Kahan): w = c*d rounded, e = exact error of w
-__device__ __forceinline__ float diff_of_products(float a, float b, float c, float d)
+template <class V>
+__device__ __forceinline__ V diff_of_products(V a, V b, V c, V d)
 {
-    const float w = c * d;
-    const float e = fmaf(-c, d, w);
-    const float f = fmaf(a, b, -w);
-    return f + e;
+    using namespace lp;
+    const V w = mul(c, d);
+    const V e = fma(neg(c), d, w);
+    const V f = fma(a, b, neg(w));
+    return add(f, e);
 }
 
-__device__ __forceinline__ EPair eq2_energy(const float m[9])
+// The three invariants of M the cubic and the quartic are built from: c2 = |M|_F^2, c1 = |cof M|_F^2, d = det M.
+template <class V> struct EqInvariants { V c2, c1, d; };
+
+template <class V>
+__device__ __forceinline__ EqInvariants<V> eq2_invariants(const V m[9])
 {
+    using namespace lp;
     // c2 = |M|_F^2
-    float c2 = m[0] * m[0];
+    V c2 = mul(m[0], m[0]);
 #pragma unroll
-    for (int i = 1; i < 9; ++i) c2 = fmaf(m[i], m[i], c2);
+    for (int i = 1; i < 9; ++i) c2 = fma(m[i], m[i], c2);
 
     // cofactor rows: C0 = r1 x r2, C1 = r2 x r0, C2 = r0 x r1.  The first row, which det M is expanded along,
     // uses Kahan's FMA difference of products (error ~1 ulp of the result): for a rank-deficient M the
     // cofactors are pure cancellation and det M must inherit their RELATIVE accuracy, because it enters E
     // under a square root (2 d / s1 below).  The other six only enter through c1 = sum C^2, where an
     // absolute error of eps |M|^2 is harmless.
-    float C[9];
+    V C[9];
     C[0] = diff_of_products(m[4], m[8], m[5], m[7]);
     C[1] = diff_of_products(m[5], m[6], m[3], m[8]);
     C[2] = diff_of_products(m[3], m[7], m[4], m[6]);
-    C[3] = fmaf(m[7], m[2], -(m[8] * m[1]));
-    C[4] = fmaf(m[8], m[0], -(m[6] * m[2]));
-    C[5] = fmaf(m[6], m[1], -(m[7] * m[0]));
-    C[6] = fmaf(m[1], m[5], -(m[2] * m[4]));
-    C[7] = fmaf(m[2], m[3], -(m[0] * m[5]));
-    C[8] = fmaf(m[0], m[4], -(m[1] * m[3]));
-    float c1 = C[0] * C[0];
+    C[3] = fma(m[7], m[2], neg(mul(m[8], m[1])));
+    C[4] = fma(m[8], m[0], neg(mul(m[6], m[2])));
+    C[5] = fma(m[6], m[1], neg(mul(m[7], m[0])));
+    C[6] = fma(m[1], m[5], neg(mul(m[2], m[4])));
+    C[7] = fma(m[2], m[3], neg(mul(m[0], m[5])));
+    C[8] = fma(m[0], m[4], neg(mul(m[1], m[3])));
+    V c1 = mul(C[0], C[0]);
 #pragma unroll
-    for (int i = 1; i < 9; ++i) c1 = fmaf(C[i], C[i], c1);
-    const float d = fmaf(m[2], C[2], fmaf(m[1], C[1], m[0] * C[0]));     // det M; its sign is S
+    for (int i = 1; i < 9; ++i) c1 = fma(C[i], C[i], c1);
+    EqInvariants<V> r;
+    r.c2 = c2;
+    r.c1 = c1;
+    r.d = fma(m[2], C[2], fma(m[1], C[1], mul(m[0], C[0])));           // det M; its sign is S
+    return r;
+}
 
-    EPair r;
-
+// E from the invariants (the serial, latency-bound half of the closed form; the tensor-core engine overlaps it
+// with the next tile's accumulator loads)
+template <class V>
+__device__ __forceinline__ EPairT<V> eq2_energy(const EqInvariants<V> inv)
+{
+    using namespace lp;
+    const V c2 = inv.c2, c1 = inv.c1, d = inv.d;
     // largest root of the cubic, Viete:  l1 = q + 2 sqrt(p) cos(acos(rr / p^1.5) / 3)
-    const float q = c2 * (1.0f / 3.0f);
-    float pp = fmaf(c2, c2, -3.0f * c1) * (1.0f / 9.0f);
-    pp = pp > 0.0f ? pp : 0.0f;
-    const float d2 = d * d;
-    const float rr = fmaf(27.0f, d2, c2 * fmaf(2.0f * c2, c2, -9.0f * c1)) * (1.0f / 54.0f);
-    const float sp = sqrt_fast(pp);
-    float ratio = pp > 0.0f ? rr * rcp_fast(pp * sp) : 1.0f;
-    ratio = fminf(1.0f, fmaxf(-1.0f, ratio));
-    const float theta = acos_fast(ratio) * (1.0f / 3.0f);              // in [0, pi/3]
-    float l1 = fmaf(2.0f * sp, cos_fast(theta), q);
-    l1 = fmaxf(l1, q);                                                  // l1 >= trace/3 always
-    const float is1 = rsqrt_fast(l1);
-    const float s1 = l1 * is1;
-    const float inv1 = is1 * is1;
+    const V q = mul(c2, splat<V>(1.0f / 3.0f));
+    V pp = mul(fma(c2, c2, mul(splat<V>(-3.0f), c1)), splat<V>(1.0f / 9.0f));
+    pp = map(pp, [](float t) { return t > 0.0f ? t : 0.0f; });
+    const V d2 = mul(d, d);
+    const V rr = mul(fma(splat<V>(27.0f), d2, mul(c2, fma(mul(splat<V>(2.0f), c2), c2, mul(splat<V>(-9.0f), c1)))),
+                     splat<V>(1.0f / 54.0f));
+    const V sp = map(pp, [](float t) { return sqrt_fast(t); });
+    const V ps = mul(pp, sp);
+    V ratio = zip3(pp, rr, ps, [](float p_, float r_, float ps_) { return p_ > 0.0f ? r_ * rcp_fast(ps_) : 1.0f; });
+    ratio = map(ratio, [](float t) { return fminf(1.0f, fmaxf(-1.0f, t)); });
+    const V theta = mul(acos_fast(ratio), splat<V>(1.0f / 3.0f));     // in [0, pi/3]
+    V l1 = fma(mul(splat<V>(2.0f), sp), map(theta, [](float t) { return cos_fast(t); }), q);
+    l1 = zip(l1, q, [](float a_, float b_) { return fmaxf(a_, b_); }); // l1 >= trace/3 always
+    const V is1 = map(l1, [](float t) { return rsqrt_fast(t); });
+    const V s1 = mul(l1, is1);
+    const V inv1 = mul(is1, is1);
     // deflation: (s2 + S s3)^2 = (c1 - d^2/l1)/l1 + 2 d / s1
-    const float w2 = fmaf(2.0f * d, is1, (c1 - d2 * inv1) * inv1);
-    const float w = sqrt_fast(w2 > 0.0f ? w2 : 0.0f);
-    const float E0 = s1 + w;
+    const V w2 = fma(mul(splat<V>(2.0f), d), is1, mul(fma(neg(d2), inv1, c1), inv1));
+    const V w = map(w2, [](float t) { return sqrt_fast(t > 0.0f ? t : 0.0f); });
+    const V E0 = add(s1, w);
 
     // one Newton step on the quartic; skipped where f' is tiny against E^3 (s2 + S s3 -> 0: the
     // quartic's roots pair up and the deflated value above is the well-conditioned one)
-    const float t = fmaf(E0, E0, -c2);
-    const float f = fmaf(t, t, fmaf(-8.0f * d, E0, -4.0f * c1));
-    const float fp = fmaf(4.0f * E0, t, -8.0f * d);
+    const V t = fma(E0, E0, neg(c2));
+    const V f = fma(t, t, fma(mul(splat<V>(-8.0f), d), E0, mul(splat<V>(-4.0f), c1)));
+    const V fp = fma(mul(splat<V>(4.0f), E0), t, mul(splat<V>(-8.0f), d));
+    const V lim = mul(mul(splat<V>(1e-3f), E0), mul(E0, E0));
     // M == 0 (L = 1, or every atom on the centroid): E = 0 (the lines above then hold 0 * inf, selected away
     // here, so the function stays branch-free); a NaN in M gives c2 = NaN and passes through as NaN
-    const bool nonzero = c2 > 1e-30f;
-    r.E0 = nonzero ? E0 : c2 * 0.0f;
-    r.delta = (nonzero && fp > 1e-3f * E0 * E0 * E0) ? f * rcp_fast(fp) : 0.0f;
+    EPairT<V> r;
+    r.E0 = zip(c2, E0, [](float c2_, float e_) { return c2_ > 1e-30f ? e_ : c2_ * 0.0f; });
+    const V step = zip3(f, fp, lim, [](float f_, float fp_, float lim_) { return fp_ > lim_ ? f_ * rcp_fast(fp_) : 0.0f; });
+    r.delta = zip(c2, step, [](float c2_, float s_) { return c2_ > 1e-30f ? s_ : 0.0f; });
     return r;
+}
+
+template <class V>
+__device__ __forceinline__ EPairT<V> eq2_energy(const V m[9])
+{
+    return eq2_energy(eq2_invariants(m));
 }
 
 // The last line of eq. 2 for a pair (i, j) whose models carry power-of-two scales 2^ei, 2^ej:
@@ -137,14 +198,15 @@ __device__ __forceinline__ float eq2_crmsd(const float m[9], float Shi_i, float 
 // pw = 2^e (|e| <= 30, so every product below stays far inside the fp32 range):  with pp = pw_i pw_j,
 //   L c^2 = (T_i - E pp) + (T_j - E pp);   E0 pp is exact, and each difference is exact by Sterbenz when the
 // models are similar.  c = sqrt(max(0, .) / L) by the MUFU square root (relative error 2^-22 << 1e-3 A).
-__device__ __forceinline__ float eq2_finish(const EPair e, float Thi_i, float Tlo_i, float pw_i, float Thi_j,
-                                            float Tlo_j, float pw_j, float invL)
+template <class V>
+__device__ __forceinline__ V eq2_finish(const EPairT<V> e, V Thi_i, V Tlo_i, V pw_i, V Thi_j, V Tlo_j, V pw_j, float invL)
 {
-    const float pp = pw_i * pw_j;
-    const float E0p = e.E0 * pp;
-    float res = ((Thi_i - E0p) + (Thi_j - E0p)) + fmaf(2.0f * e.delta, pp, Tlo_i + Tlo_j);
-    res = res < 0.0f ? 0.0f : res;                                      // clamp (NaN stays NaN)
-    return sqrt_fast(res * invL);
+    using namespace lp;
+    const V pp = mul(pw_i, pw_j);
+    const V E0p = mul(e.E0, pp);
+    const V res = add(add(sub(Thi_i, E0p), sub(Thi_j, E0p)), fma(mul(splat<V>(2.0f), e.delta), pp, add(Tlo_i, Tlo_j)));
+    const V sc = mul(res, splat<V>(invL));
+    return map(sc, [](float t) { return sqrt_fast(t < 0.0f ? 0.0f : t); });      // clamp (NaN stays NaN)
 }
 
 }  // namespace clusco

@@ -300,6 +300,25 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         int64_t curI = -1, i = 0, rowoff = 0;
         bool row_ok = false;
         PairStat si = {0.0f, 0.0f, 1.0f, 0.0f};
+        // The closed form of a tile is evaluated in two halves, software-pipelined over the team's tiles: the
+        // invariants (c2, c1, det) right after the accumulators are read, the serial root-finding half (Viete,
+        // Newton, finish, store) one tile later, between the issue of the next tile's TMEM loads and their
+        // completion -- two independent dependency chains per thread instead of one.
+        struct Pending {
+            EqInvariants<float2> inv;
+            float Thi, Tlo, pw;                  // row model
+            float2 Thj, Tlj, pwj;                // the two column models
+            float* dst;                          // out + rowoff + j0
+            bool ok0, ok1;
+        } pend;
+        bool have_pend = false;
+        auto finish_pending = [&]() {
+            const float2 c = eq2_finish(eq2_energy(pend.inv), make_float2(pend.Thi, pend.Thi),
+                                        make_float2(pend.Tlo, pend.Tlo), make_float2(pend.pw, pend.pw), pend.Thj,
+                                        pend.Tlj, pend.pwj, P.invLk);
+            if (pend.ok0) pend.dst[0] = c.x;
+            if (pend.ok1) pend.dst[4] = c.y;
+        };
         for (uint32_t n = team; n < ntiles; n += 2) {
             if (I != curI) {                                     // per-row quantities (warp-uniform branch)
                 curI = I;
@@ -315,13 +334,13 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             ptx::mbar_wait(ACC_FULL(buf), (n >> 1) & 1);
             ptx::tc_fence_after();
             const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16) + buf * I8_ACC_COLS + half * 8;
-            // m[e][3p+q]: pair (row model r, column model c4 + 4e + 8 half), Gram sums in units of 2^46
-            float m[2][9];
+            // m[3p+q] = (.x, .y): pairs (row model r, column model c4 + 8 half) and (.., + 4); Gram sums in units
+            // of 2^46.  The two pairs of a thread go through the closed form together, on packed fp32 arithmetic.
+            float2 m[9];
 #if defined(I8_EXPERIMENT) && I8_EXPERIMENT >= 3              // developer switch: no TMEM loads, no arithmetic
 #pragma unroll
-            for (int e = 0; e < 2; ++e)
-#pragma unroll
-                for (int q = 0; q < 9; ++q) m[e][q] = (float)(n + q);
+            for (int q = 0; q < 9; ++q) m[q] = make_float2((float)(n + q), (float)(n + q + 1));
+            if (have_pend) finish_pending();
 #else
             {
                 // levels 1 and 2 first: T = 2^8 V1 + V2 fits int32 (|T| < 2^31 for L <= 256 because |d0| <= 127)
@@ -333,20 +352,17 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                         ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 48 + 16 * q, v1[q][h]);
                         ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 96 + 16 * q, v2[q][h]);
                     }
+                if (have_pend) finish_pending();                 // previous tile's serial half, under the load latency
                 ptx::tmem_ld_wait();
-                int32_t T[2][9];
+                const float2 s30 = make_float2(0x1p-30f, 0x1p-30f);
 #pragma unroll
-                for (int q = 0; q < 3; ++q)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        T[e][0 + q] = ((int32_t)v1[q][0][e] << 8) + (int32_t)v2[q][0][e];
-                        T[e][3 + q] = ((int32_t)v1[q][0][2 + e] << 8) + (int32_t)v2[q][0][2 + e];
-                        T[e][6 + q] = ((int32_t)v1[q][1][e] << 8) + (int32_t)v2[q][1][e];
-                    }
-#pragma unroll
-                for (int e = 0; e < 2; ++e)
-#pragma unroll
-                    for (int q = 0; q < 9; ++q) m[e][q] = (float)T[e][q] * 0x1p-30f;
+                for (int q = 0; q < 3; ++q) {
+                    // register slots of a 16x256b load: [0,1] = lane r (h = 0: p = 0, h = 1: p = 2), [2,3] = lane r + 8 (p = 1)
+                    auto T = [&](int h, int e) { return (float)(((int32_t)v1[q][h][e] << 8) + (int32_t)v2[q][h][e]); };
+                    m[0 + q] = __fmul2_rn(make_float2(T(0, 0), T(0, 1)), s30);
+                    m[3 + q] = __fmul2_rn(make_float2(T(0, 2), T(0, 3)), s30);
+                    m[6 + q] = __fmul2_rn(make_float2(T(1, 0), T(1, 1)), s30);
+                }
             }
             {
                 uint32_t v0[3][2][4];
@@ -355,14 +371,14 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
 #pragma unroll
                     for (int h = 0; h < 2; ++h) ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 16 * q, v0[q][h]);
                 ptx::tmem_ld_wait();
+                const float2 s14 = make_float2(0x1p-14f, 0x1p-14f);
 #pragma unroll
-                for (int q = 0; q < 3; ++q)
-#pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        m[e][0 + q] = fmaf((float)(int32_t)v0[q][0][e], 0x1p-14f, m[e][0 + q]);
-                        m[e][3 + q] = fmaf((float)(int32_t)v0[q][0][2 + e], 0x1p-14f, m[e][3 + q]);
-                        m[e][6 + q] = fmaf((float)(int32_t)v0[q][1][e], 0x1p-14f, m[e][6 + q]);
-                    }
+                for (int q = 0; q < 3; ++q) {
+                    auto F = [&](int h, int e) { return (float)(int32_t)v0[q][h][e]; };
+                    m[0 + q] = __ffma2_rn(make_float2(F(0, 0), F(0, 1)), s14, m[0 + q]);
+                    m[3 + q] = __ffma2_rn(make_float2(F(0, 2), F(0, 3)), s14, m[3 + q]);
+                    m[6 + q] = __ffma2_rn(make_float2(F(1, 0), F(1, 1)), s14, m[6 + q]);
+                }
             }
 #endif
             // the accumulator buffer is free again
@@ -371,21 +387,24 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
 
 #if defined(I8_EXPERIMENT) && (I8_EXPERIMENT == 1 || I8_EXPERIMENT >= 3)   // developer switch: no eq. 2 arithmetic
-            const float c0 = m[0][0] + m[0][4] + m[0][8], c1 = m[1][0] + m[1][4] + m[1][8];
-            if (row_ok && j0 < P.N && j0 > i) P.out[rowoff + j0] = c0 + si.Thi + sj0.Thi;
-            if (row_ok && j0 + 4 < P.N && j0 + 4 > i) P.out[rowoff + j0 + 4] = c1 + sj1.Thi;
+            pend.inv.c2 = m[0]; pend.inv.c1 = m[4]; pend.inv.d = m[8];
 #else
-            // both pairs are evaluated branch-free (their chains interleave); masked pairs are simply not stored
-            const float c0 = eq2_finish(eq2_energy(m[0]), si.Thi, si.Tlo, si.pw, sj0.Thi, sj0.Tlo, sj0.pw, P.invLk);
-            const float c1 = eq2_finish(eq2_energy(m[1]), si.Thi, si.Tlo, si.pw, sj1.Thi, sj1.Tlo, sj1.pw, P.invLk);
-            if (row_ok && j0 < P.N && j0 > i) P.out[rowoff + j0] = c0;
-            if (row_ok && j0 + 4 < P.N && j0 + 4 > i) P.out[rowoff + j0 + 4] = c1;
+            pend.inv = eq2_invariants(m);
 #endif
+            pend.Thi = si.Thi; pend.Tlo = si.Tlo; pend.pw = si.pw;
+            pend.Thj = make_float2(sj0.Thi, sj1.Thi);
+            pend.Tlj = make_float2(sj0.Tlo, sj1.Tlo);
+            pend.pwj = make_float2(sj0.pw, sj1.pw);
+            pend.dst = P.out + rowoff + j0;
+            pend.ok0 = row_ok && j0 < P.N && j0 > i;             // masked pairs are simply not stored
+            pend.ok1 = row_ok && j0 + 4 < P.N && j0 + 4 > i;
+            have_pend = true;
             // advance two tiles
 #pragma unroll
             for (int s = 0; s < 2; ++s)
                 if (++J >= Tc) { ++I; J = 2 * I; }
         }
+        if (have_pend) finish_pending();
     }
 #if defined(I8_EXPERIMENT) && I8_EXPERIMENT == 6
 done:
