@@ -116,12 +116,22 @@ int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N,
                             float* out, void* stream);
 
 /*
- * Host-buffer convenience calls (blocking): allocate device memory, copy in, compute, copy the
- * result back, free.  coords_host / out_host are ordinary (preferably pinned) host pointers.
+ * Host-buffer calls (blocking; the end-to-end path): coords_host / native_host / out_host are ordinary host
+ * pointers -- pinned (page-locked) memory lets the transfers overlap the kernels, pageable memory works
+ * but serialises.  Device scratch (inputs, result, workspace) is taken from a library-owned
+ * stream-ordered memory pool that is KEPT between calls, so a repeated call pays no allocation;
+ * transfers run on the library's own copy stream:
+ *   all-pairs:   H2D coords -> prepare -> for each of 8 row chunks of equal pair count
+ *                (clusco_partition_rows): compute chunk k | D2H chunk k-1;
+ *   one-vs-all:  the models go up in ~64 MB chunks, each scored as soon as it has landed.
+ * One host call runs at a time per process (internal lock).  Errors: as the device calls, plus
+ * CLUSCO_ERR_CUDA for allocation / copy failures (nothing is leaked; the streams are drained first).
  */
 int clusco_crmsd_allpairs_host(const float* coords_host, int64_t N, int32_t L, float* out_host);
 int clusco_crmsd_one_vs_all_host(const float* native_host, const float* coords_host, int64_t N,
                                  int32_t L, float* out_host);
+/* Returns the pool kept by the *_host calls to the driver and destroys their streams (all devices). */
+int clusco_host_release(void);
 
 /*
  * Balanced row partition for `parts` ranks: writes parts+1 boundaries (multiples of 128, first 0,

@@ -25,6 +25,7 @@ EXPORTS = (
     "clusco_crmsd_allpairs_workspace", "clusco_crmsd_allpairs", "clusco_crmsd_allpairs_ex",
     "clusco_crmsd_one_vs_all", "clusco_crmsd_allpairs_host", "clusco_crmsd_one_vs_all_host",
     "clusco_partition_rows", "clusco_engine_supported", "clusco_allpairs_prepare", "clusco_allpairs_compute",
+    "clusco_host_release",
 )
 
 
@@ -211,6 +212,11 @@ def clusco_crmsd_one_vs_all_host(native_host, coords_host, out_host=None):
     _check(load().clusco_crmsd_one_vs_all_host(_ptr(native_host), _ptr(coords_host), N, L, _ptr(out_host)),
            "clusco_crmsd_one_vs_all_host")
     return out_host
+
+
+def clusco_host_release():
+    """Return the device memory pool kept by the *_host calls to the driver."""
+    _check(load().clusco_host_release(), "clusco_host_release")
 
 
 def clusco_partition_rows(N: int, parts: int):

@@ -3,6 +3,8 @@
 #include <math.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "common.cuh"
 #include "epilogue.cuh"
 #include "gram_ffma.cuh"
@@ -190,7 +192,7 @@ int clusco_crmsd_allpairs(const float* coords, int64_t N, int32_t L, float* out,
                                     CLUSCO_ENGINE_AUTO, stream);
 }
 
-// scratch for the centred native lives in a small per-call device allocation ordered on the stream
+// one launch, no scratch: every CTA centres the native into its own shared memory
 int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream)
 {
     if (N < 0 || L < 1) return CLUSCO_ERR_INVALID_ARG;
@@ -203,15 +205,6 @@ int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N,
     const size_t nat_bytes = (size_t)L * sizeof(float4);
     if (nat_bytes > 200 * 1024) return CLUSCO_ERR_INVALID_ARG;        // L <= 12800 atoms
     if (!aligned16(coords)) return CLUSCO_ERR_INVALID_ARG;
-    const size_t natc_sz = (size_t)round_up((int64_t)nat_bytes, 256);
-    const size_t natq_sz = (size_t)round_up((int64_t)((L + 3) / 4) * OVA_NATQ_FLOATS * 4, 256);
-    char* scratch = nullptr;
-    CLUSCO_CUDA_TRY(cudaMallocAsync((void**)&scratch, natc_sz + natq_sz + 256, s));
-    float4* natc = (float4*)scratch;
-    float* natq = (float*)(scratch + natc_sz);
-    NativeStat* nstat = (NativeStat*)(scratch + natc_sz + natq_sz);
-    native_prep_kernel<<<1, 256, 0, s>>>(native, L, natc, natq, nstat);
-    CLUSCO_CUDA_TRY(cudaGetLastError());
     const int64_t n_blocks32 = (N + 31) / 32;
     int warps = 0, stages = 0;
     if (ova_stream_config(L, &warps, &stages)) {
@@ -224,27 +217,91 @@ int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N,
     do {                                                                                                               \
         CLUSCO_CUDA_TRY(cudaFuncSetAttribute(one_vs_all_stream_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
                                              (int)smem));                                                              \
-        one_vs_all_stream_kernel<V><<<(unsigned)grid, warps * 32, smem, s>>>(natq, nstat, coords, N, L,                \
-                                                                             1.0f / (float)L, stages, out);            \
+        one_vs_all_stream_kernel<V><<<(unsigned)grid, warps * 32, smem, s>>>(native, coords, N, L, 1.0f / (float)L,    \
+                                                                             stages, out);                             \
     } while (0)
         if (vec == 4) OVA_LAUNCH(4); else if (vec == 2) OVA_LAUNCH(2); else OVA_LAUNCH(1);
 #undef OVA_LAUNCH
     } else {
-        static thread_local size_t smem_set = 0;
-        if (nat_bytes > 48 * 1024 && nat_bytes > smem_set) {
-            CLUSCO_CUDA_TRY(cudaFuncSetAttribute(one_vs_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                 (int)nat_bytes));
-            smem_set = nat_bytes;
-        }
+        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(one_vs_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)nat_bytes));
         int64_t grid = (n_blocks32 + OVA_WARPS - 1) / OVA_WARPS;
-        const int64_t cap = (int64_t)sms * 8;
+        const int64_t cap = (int64_t)sms * 4;
         if (grid > cap) grid = cap;
-        one_vs_all_kernel<<<(unsigned)grid, OVA_WARPS * 32, nat_bytes, s>>>(natc, nstat, coords, N, L,
-                                                                           1.0f / (float)L, out);
+        one_vs_all_kernel<<<(unsigned)grid, OVA_WARPS * 32, nat_bytes, s>>>(native, coords, N, L, 1.0f / (float)L, out);
     }
     CLUSCO_CUDA_TRY(cudaGetLastError());
-    CLUSCO_CUDA_TRY(cudaFreeAsync(scratch, s));
     return CLUSCO_OK;
+}
+
+// ---- host-buffer calls ---------------------------------------------------------------------------------
+// Device scratch comes from a library-owned stream-ordered memory pool (one per device, kept between calls so
+// that repeated calls pay no allocation; clusco_host_release() returns it to the driver), and the transfers
+// run on their own stream, overlapped with the kernels chunk by chunk.
+namespace {
+struct HostCtx {
+    cudaMemPool_t pool = nullptr;
+    cudaStream_t compute = nullptr, copy = nullptr;
+};
+std::mutex g_host_mu;
+HostCtx g_host[64];
+
+int host_ctx(HostCtx** out)
+{
+    int dev = 0;
+    CLUSCO_CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return CLUSCO_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_host_mu);
+    HostCtx& c = g_host[dev];
+    if (!c.pool) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        CLUSCO_CUDA_TRY(cudaMemPoolCreate(&c.pool, &props));
+        uint64_t keep = UINT64_MAX;                          // keep freed blocks for the next call
+        CLUSCO_CUDA_TRY(cudaMemPoolSetAttribute(c.pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        CLUSCO_CUDA_TRY(cudaStreamCreateWithFlags(&c.compute, cudaStreamNonBlocking));
+        CLUSCO_CUDA_TRY(cudaStreamCreateWithFlags(&c.copy, cudaStreamNonBlocking));
+    }
+    *out = &c;
+    return CLUSCO_OK;
+}
+
+// first error wins; later CUDA calls are still made so that every stream is drained before returning
+struct ErrLatch {
+    int st = CLUSCO_OK;
+    void cuda(cudaError_t e)
+    {
+        if (e != cudaSuccess && st == CLUSCO_OK) {
+            g_last_cuda_error = (int)e;
+            st = CLUSCO_ERR_CUDA;
+        }
+    }
+    void status(int s)
+    {
+        if (s != CLUSCO_OK && st == CLUSCO_OK) st = s;
+    }
+    bool ok() const { return st == CLUSCO_OK; }
+};
+}  // namespace
+
+int clusco_host_release(void)
+{
+    std::lock_guard<std::mutex> lock(g_host_mu);
+    int st = CLUSCO_OK;
+    for (HostCtx& c : g_host) {
+        if (!c.pool) continue;
+        cudaStreamSynchronize(c.compute);
+        cudaStreamSynchronize(c.copy);
+        cudaStreamDestroy(c.compute);
+        cudaStreamDestroy(c.copy);
+        if (cudaMemPoolDestroy(c.pool) != cudaSuccess) st = CLUSCO_ERR_CUDA;
+        c = HostCtx();
+    }
+    return st;
 }
 
 int clusco_crmsd_allpairs_host(const float* coords_host, int64_t N, int32_t L, float* out_host)
@@ -252,37 +309,56 @@ int clusco_crmsd_allpairs_host(const float* coords_host, int64_t N, int32_t L, f
     if (N < 0 || L < 1) return CLUSCO_ERR_INVALID_ARG;
     if (N < 2) return CLUSCO_OK;
     if (!coords_host || !out_host) return CLUSCO_ERR_INVALID_ARG;
+    int st = check_device(nullptr);
+    if (st != CLUSCO_OK) return st;
+    HostCtx* ctx = nullptr;
+    st = host_ctx(&ctx);
+    if (st != CLUSCO_OK) return st;
+    std::lock_guard<std::mutex> lock(g_host_mu);             // one host call at a time per process
     const size_t in_bytes = (size_t)N * L * 3 * sizeof(float);
     const size_t n_pairs = (size_t)N * (size_t)(N - 1) / 2;
     const size_t ws_bytes = clusco_crmsd_allpairs_workspace(N, L);
+    cudaStream_t sc = ctx->compute, sx = ctx->copy;
     float *d_in = nullptr, *d_out = nullptr;
     void* d_ws = nullptr;
-    cudaStream_t s;
-    CLUSCO_CUDA_TRY(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
-    int st = CLUSCO_OK;
-    cudaError_t e;
-    if ((e = cudaMalloc((void**)&d_in, in_bytes)) != cudaSuccess ||
-        (e = cudaMalloc((void**)&d_out, n_pairs * sizeof(float))) != cudaSuccess ||
-        (e = cudaMalloc(&d_ws, ws_bytes)) != cudaSuccess) {
-        g_last_cuda_error = (int)e;
-        st = CLUSCO_ERR_CUDA;
+    ErrLatch err;
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_in, in_bytes, ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_out, n_pairs * sizeof(float), ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync(&d_ws, ws_bytes, ctx->pool, sc));
+    // rows are cut into chunks of equal pair count; chunk k is copied back while chunk k+1 is computed
+    constexpr int MAX_CHUNKS = 8;
+    int64_t bounds[MAX_CHUNKS + 1];
+    const int chunks = n_pairs * sizeof(float) >= ((size_t)8 << 20) ? MAX_CHUNKS : 1;
+    err.status(clusco_partition_rows(N, chunks, bounds));
+    cudaEvent_t ev[MAX_CHUNKS];
+    int n_ev = 0;
+    if (err.ok()) {
+        err.cuda(cudaMemcpyAsync(d_in, coords_host, in_bytes, cudaMemcpyHostToDevice, sc));
+        err.status(clusco_allpairs_prepare(d_in, N, L, d_ws, ws_bytes, CLUSCO_ENGINE_AUTO, (void*)sc));
     }
-    if (st == CLUSCO_OK && (e = cudaMemcpyAsync(d_in, coords_host, in_bytes, cudaMemcpyHostToDevice, s)) != cudaSuccess) {
-        g_last_cuda_error = (int)e;
-        st = CLUSCO_ERR_CUDA;
+    for (int k = 0; k < chunks && err.ok(); ++k) {
+        const int64_t lo = bounds[k], hi = bounds[k + 1];
+        if (hi <= lo) continue;
+        const int64_t off = packed_index(lo, lo + 1, N);
+        const int64_t end = hi >= N ? (int64_t)n_pairs : packed_index(hi, hi + 1, N);
+        if (end <= off) continue;
+        err.status(clusco_allpairs_compute(N, L, lo, hi, d_out + off, d_ws, ws_bytes, CLUSCO_ENGINE_AUTO, (void*)sc));
+        if (!err.ok()) break;
+        err.cuda(cudaEventCreateWithFlags(&ev[n_ev], cudaEventDisableTiming));
+        if (!err.ok()) break;
+        ++n_ev;
+        err.cuda(cudaEventRecord(ev[n_ev - 1], sc));
+        err.cuda(cudaStreamWaitEvent(sx, ev[n_ev - 1], 0));
+        err.cuda(cudaMemcpyAsync(out_host + off, d_out + off, (size_t)(end - off) * sizeof(float),
+                                 cudaMemcpyDeviceToHost, sx));
     }
-    if (st == CLUSCO_OK) st = clusco_crmsd_allpairs(d_in, N, L, d_out, d_ws, ws_bytes, (void*)s);
-    if (st == CLUSCO_OK &&
-        ((e = cudaMemcpyAsync(out_host, d_out, n_pairs * sizeof(float), cudaMemcpyDeviceToHost, s)) != cudaSuccess ||
-         (e = cudaStreamSynchronize(s)) != cudaSuccess)) {
-        g_last_cuda_error = (int)e;
-        st = CLUSCO_ERR_CUDA;
-    }
-    cudaFree(d_in);
-    cudaFree(d_out);
-    cudaFree(d_ws);
-    cudaStreamDestroy(s);
-    return st;
+    err.cuda(cudaStreamSynchronize(sx));
+    err.cuda(cudaStreamSynchronize(sc));
+    for (int k = 0; k < n_ev; ++k) cudaEventDestroy(ev[k]);
+    if (d_in) cudaFreeAsync(d_in, sc);
+    if (d_out) cudaFreeAsync(d_out, sc);
+    if (d_ws) cudaFreeAsync(d_ws, sc);
+    return err.st;
 }
 
 int clusco_crmsd_one_vs_all_host(const float* native_host, const float* coords_host, int64_t N, int32_t L,
@@ -291,32 +367,49 @@ int clusco_crmsd_one_vs_all_host(const float* native_host, const float* coords_h
     if (N < 0 || L < 1) return CLUSCO_ERR_INVALID_ARG;
     if (N == 0) return CLUSCO_OK;
     if (!native_host || !coords_host || !out_host) return CLUSCO_ERR_INVALID_ARG;
-    const size_t in_bytes = (size_t)N * L * 3 * sizeof(float), nat_bytes = (size_t)L * 3 * sizeof(float);
+    int st = check_device(nullptr);
+    if (st != CLUSCO_OK) return st;
+    HostCtx* ctx = nullptr;
+    st = host_ctx(&ctx);
+    if (st != CLUSCO_OK) return st;
+    std::lock_guard<std::mutex> lock(g_host_mu);
+    const size_t model_bytes = (size_t)L * 3 * sizeof(float);
+    cudaStream_t sc = ctx->compute, sx = ctx->copy;
     float *d_in = nullptr, *d_nat = nullptr, *d_out = nullptr;
-    cudaStream_t s;
-    CLUSCO_CUDA_TRY(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking));
-    int st = CLUSCO_OK;
-    cudaError_t e;
-    if ((e = cudaMalloc((void**)&d_in, in_bytes)) != cudaSuccess ||
-        (e = cudaMalloc((void**)&d_nat, nat_bytes)) != cudaSuccess ||
-        (e = cudaMalloc((void**)&d_out, (size_t)N * sizeof(float))) != cudaSuccess ||
-        (e = cudaMemcpyAsync(d_nat, native_host, nat_bytes, cudaMemcpyHostToDevice, s)) != cudaSuccess ||
-        (e = cudaMemcpyAsync(d_in, coords_host, in_bytes, cudaMemcpyHostToDevice, s)) != cudaSuccess) {
-        g_last_cuda_error = (int)e;
-        st = CLUSCO_ERR_CUDA;
+    ErrLatch err;
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_in, (size_t)N * model_bytes, ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_nat, model_bytes, ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_out, (size_t)N * sizeof(float), ctx->pool, sc));
+    // the models go up in chunks (a multiple of 32 models, about 64 MB) on the copy stream; each chunk is
+    // scored as soon as it has landed, so the kernels hide behind the transfer
+    int64_t per = ((int64_t)(64 << 20) / (int64_t)model_bytes) / 32 * 32;
+    if (per < 32) per = 32;
+    const int64_t chunks = (N + per - 1) / per;
+    cudaEvent_t ready = nullptr, alloc_done = nullptr;
+    err.cuda(cudaEventCreateWithFlags(&ready, cudaEventDisableTiming));
+    err.cuda(cudaEventCreateWithFlags(&alloc_done, cudaEventDisableTiming));
+    if (err.ok()) {
+        err.cuda(cudaMemcpyAsync(d_nat, native_host, model_bytes, cudaMemcpyHostToDevice, sc));
+        err.cuda(cudaEventRecord(alloc_done, sc));                    // the pool blocks are ordered on sc
+        err.cuda(cudaStreamWaitEvent(sx, alloc_done, 0));
     }
-    if (st == CLUSCO_OK) st = clusco_crmsd_one_vs_all(d_nat, d_in, N, L, d_out, (void*)s);
-    if (st == CLUSCO_OK &&
-        ((e = cudaMemcpyAsync(out_host, d_out, (size_t)N * sizeof(float), cudaMemcpyDeviceToHost, s)) != cudaSuccess ||
-         (e = cudaStreamSynchronize(s)) != cudaSuccess)) {
-        g_last_cuda_error = (int)e;
-        st = CLUSCO_ERR_CUDA;
+    for (int64_t k = 0; k < chunks && err.ok(); ++k) {
+        const int64_t m0 = k * per, cnt = (m0 + per <= N ? per : N - m0);
+        err.cuda(cudaMemcpyAsync(d_in + m0 * (int64_t)L * 3, coords_host + m0 * (int64_t)L * 3, (size_t)cnt * model_bytes,
+                                 cudaMemcpyHostToDevice, sx));
+        err.cuda(cudaEventRecord(ready, sx));
+        err.cuda(cudaStreamWaitEvent(sc, ready, 0));
+        err.status(clusco_crmsd_one_vs_all(d_nat, d_in + m0 * (int64_t)L * 3, cnt, L, d_out + m0, (void*)sc));
     }
-    cudaFree(d_in);
-    cudaFree(d_nat);
-    cudaFree(d_out);
-    cudaStreamDestroy(s);
-    return st;
+    if (err.ok()) err.cuda(cudaMemcpyAsync(out_host, d_out, (size_t)N * sizeof(float), cudaMemcpyDeviceToHost, sc));
+    err.cuda(cudaStreamSynchronize(sx));
+    err.cuda(cudaStreamSynchronize(sc));
+    if (ready) cudaEventDestroy(ready);
+    if (alloc_done) cudaEventDestroy(alloc_done);
+    if (d_in) cudaFreeAsync(d_in, sc);
+    if (d_nat) cudaFreeAsync(d_nat, sc);
+    if (d_out) cudaFreeAsync(d_out, sc);
+    return err.st;
 }
 
 }  // extern "C"

@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             float2 Thj, Tlj, pwj;                // the two column models
             float* dst;                          // out + rowoff + j0
             bool ok0, ok1;
-        } pend;
+        } pend = {};
         bool have_pend = false;
         auto finish_pending = [&]() {
             const float2 c = eq2_finish(eq2_energy(pend.inv), make_float2(pend.Thi, pend.Thi),

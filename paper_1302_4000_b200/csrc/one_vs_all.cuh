@@ -20,19 +20,19 @@
 
 namespace clusco {
 
-// Native: centred in FP64; sum of squares as two floats.
+// Sum of squares of the centred native as two floats.
 struct NativeStat { float Shi, Slo; };
 
-// one CTA; writes natc[L] (float4: x, y, z, 0), natq (per 4-atom block and component p the twelve floats
-// [a0 a0 a1 a1] [a2 a2 a3 a3] [a0 a1 a2 a3] = the FFMA2 operand pairs of ova_block; zero padded to 4 ceil(L/4)
-// atoms) and nstat
-__global__ void __launch_bounds__(256) native_prep_kernel(const float* __restrict__ native, int32_t L,
-                                                          float4* __restrict__ natc, float* __restrict__ natq,
-                                                          NativeStat* __restrict__ nstat)
+// Every CTA centres the native itself (FP64 centroid, a1 of the hot path for the reference structure) straight
+// into its shared memory -- no scratch buffer, no extra launch; all CTAs of a launch get identical values
+// because the reduction order depends on blockDim only.  EXPANDED = false: nat_s[k] = float4 (x, y, z, 0);
+// EXPANDED = true: per 4-atom block and component p the twelve floats [a0 a0 a1 a1] [a2 a2 a3 a3] [a0 a1 a2 a3]
+// (the FFMA2 operand pairs of ova_block), zero padded to 4 ceil(L/4) atoms.  Ends with a __syncthreads().
+template <bool EXPANDED>
+__device__ __forceinline__ NativeStat ova_native_to_smem(const float* __restrict__ native, int32_t L, float* nat_s)
 {
-    __shared__ double red[3][8];
-    __shared__ double mean[3];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __shared__ double red[4][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
     double s[3] = {0.0, 0.0, 0.0};
     for (int k = threadIdx.x; k < L; k += blockDim.x) {
         s[0] += (double)native[3 * k];
@@ -45,44 +45,46 @@ __global__ void __launch_bounds__(256) native_prep_kernel(const float* __restric
         if (lane == 0) red[p][warp] = v;
     }
     __syncthreads();
-    if (threadIdx.x < 3) {
-        double v = 0.0;
-        for (int w = 0; w < 8; ++w) v += red[threadIdx.x][w];
-        mean[threadIdx.x] = v / (double)L;
-    }
-    __syncthreads();
-    double ss = 0.0;
-    const int Lp4 = (L + 3) & ~3;
-    for (int k = threadIdx.x; k < Lp4; k += blockDim.x) {
-        float ax = 0.0f, ay = 0.0f, az = 0.0f;
-        if (k < L) {
-            ax = (float)((double)native[3 * k] - mean[0]);
-            ay = (float)((double)native[3 * k + 1] - mean[1]);
-            az = (float)((double)native[3 * k + 2] - mean[2]);
-            natc[k] = make_float4(ax, ay, az, 0.0f);
-            ss += (double)ax * ax + (double)ay * ay + (double)az * az;
-        }
-        // block k/4, component p: [a0 a0 a1 a1] [a2 a2 a3 a3] [a0 a1 a2 a3]
-        float* q = natq + (k >> 2) * 36;
-        const int i = k & 3;
-        const float a[3] = {ax, ay, az};
+    double mean[3];
 #pragma unroll
-        for (int p = 0; p < 3; ++p) {
-            q[12 * p + 2 * i] = a[p];
-            q[12 * p + 2 * i + 1] = a[p];
-            q[12 * p + 8 + i] = a[p];
+    for (int p = 0; p < 3; ++p) {
+        double v = 0.0;
+        for (int w = 0; w < nw; ++w) v += red[p][w];
+        mean[p] = v / (double)L;
+    }
+    double ss = 0.0;
+    const int Lp = EXPANDED ? ((L + 3) & ~3) : L;
+    for (int k = threadIdx.x; k < Lp; k += blockDim.x) {
+        float a[3] = {0.0f, 0.0f, 0.0f};
+        if (k < L) {
+#pragma unroll
+            for (int p = 0; p < 3; ++p) {
+                a[p] = (float)((double)native[3 * k + p] - mean[p]);
+                ss += (double)a[p] * a[p];
+            }
+        }
+        if (EXPANDED) {
+            float* q = nat_s + (k >> 2) * 36;
+            const int i = k & 3;
+#pragma unroll
+            for (int p = 0; p < 3; ++p) {
+                q[12 * p + 2 * i] = a[p];
+                q[12 * p + 2 * i + 1] = a[p];
+                q[12 * p + 8 + i] = a[p];
+            }
+        } else {
+            reinterpret_cast<float4*>(nat_s)[k] = make_float4(a[0], a[1], a[2], 0.0f);
         }
     }
     ss = warp_sum(ss);
+    if (lane == 0) red[3][warp] = ss;
     __syncthreads();
-    if (lane == 0) red[0][warp] = ss;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        double v = 0.0;
-        for (int w = 0; w < 8; ++w) v += red[0][w];
-        nstat->Shi = (float)v;
-        nstat->Slo = (float)(v - (double)nstat->Shi);
-    }
+    double v = 0.0;
+    for (int w = 0; w < nw; ++w) v += red[3][w];
+    NativeStat r;
+    r.Shi = (float)v;
+    r.Slo = (float)(v - (double)r.Shi);
+    return r;
 }
 
 // eq. 2 for one model from its ten sums (nine covariance sums against the centred native + sum of squares):
@@ -110,7 +112,7 @@ __device__ __forceinline__ float ova_finish(const float mine[10], float nShi, fl
 constexpr int OVA_MPC = 4;                 // models per stage (one warp iteration), 8 lanes each
 constexpr int OVA_MAX_WARPS = 16;
 constexpr int OVA_STREAM_MAX_L = 2048;     // 2 stages of 48 L bytes + the native must fit in shared memory
-constexpr int OVA_NATQ_FLOATS = 36;        // expanded native block, see native_prep_kernel
+constexpr int OVA_NATQ_FLOATS = 36;        // expanded native block, see ova_native_to_smem
 
 // Six float2 = twelve consecutive floats (4 atoms: x0 y0 | z0 x1 | y1 z1 | x2 y2 | z2 x3 | y3 z3) of a staged
 // model; VEC = widest aligned vector (floats) every model base and block offset allows: 4 if L % 4 == 0,
@@ -179,8 +181,7 @@ __device__ __forceinline__ void ova_block(OvaAcc& acc, const float2 Bv[6], const
 
 template <int VEC>
 __global__ void __launch_bounds__(OVA_MAX_WARPS * 32, 1)
-one_vs_all_stream_kernel(const float* __restrict__ natq, const NativeStat* __restrict__ nstat,
-                         const float* __restrict__ coords, int64_t N, int32_t L, float invL, int32_t stages,
+one_vs_all_stream_kernel(const float* __restrict__ native, const float* __restrict__ coords, int64_t N, int32_t L, float invL, int32_t stages,
                          float* __restrict__ out)
 {
     extern __shared__ __align__(128) uint8_t ova_smem[];
@@ -192,12 +193,11 @@ one_vs_all_stream_kernel(const float* __restrict__ natq, const NativeStat* __res
     uint64_t* bars0 = reinterpret_cast<uint64_t*>(ring0 + (size_t)nwarps * stages * stage_bytes);
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int k = threadIdx.x; k < nblk * OVA_NATQ_FLOATS; k += blockDim.x) nat_s[k] = natq[k];
     if (lane == 0)
         for (int s = 0; s < stages; ++s) ptx::mbar_init(ptx::smem_u32(bars0 + warp * stages + s), 1);
     ptx::fence_mbar_init();
-    __syncthreads();
-    const float nShi = nstat->Shi, nSlo = nstat->Slo;
+    const NativeStat nst = ova_native_to_smem<true>(native, L, nat_s);
+    const float nShi = nst.Shi, nSlo = nst.Slo;
 
     uint8_t* ring = ring0 + (size_t)warp * stages * stage_bytes;
     const uint32_t bar = ptx::smem_u32(bars0 + warp * stages);
@@ -318,7 +318,7 @@ static inline size_t ova_stream_smem(int32_t L, int warps, int stages)
 static inline bool ova_stream_config(int32_t L, int* warps, int* stages)
 {
     if (L > OVA_STREAM_MAX_L) return false;
-    const size_t budget = 227 * 1024;
+    const size_t budget = 226 * 1024;                    // 227 KB per CTA minus the static reduction scratch
     int w = 12;
     while (w > 1 && ova_stream_smem(L, w, 2) > budget) --w;
     if (ova_stream_smem(L, w, 2) > budget) return false;
@@ -334,13 +334,11 @@ static inline bool ova_stream_config(int32_t L, int* warps, int* stages)
 constexpr int OVA_WARPS = 8;
 
 __global__ void __launch_bounds__(OVA_WARPS * 32)
-one_vs_all_kernel(const float4* __restrict__ natc, const NativeStat* __restrict__ nstat,
-                  const float* __restrict__ coords, int64_t N, int32_t L, float invL, float* __restrict__ out)
+one_vs_all_kernel(const float* __restrict__ native, const float* __restrict__ coords, int64_t N, int32_t L, float invL, float* __restrict__ out)
 {
     extern __shared__ float4 nat_s[];                     // centred native, L float4
-    for (int k = threadIdx.x; k < L; k += blockDim.x) nat_s[k] = natc[k];
-    __syncthreads();
-    const float nShi = nstat->Shi, nSlo = nstat->Slo;
+    const NativeStat nst = ova_native_to_smem<false>(native, L, reinterpret_cast<float*>(nat_s));
+    const float nShi = nst.Shi, nSlo = nst.Slo;
 
     const int lane = threadIdx.x & 31;
     const int64_t warp_g = (int64_t)blockIdx.x * OVA_WARPS + (threadIdx.x >> 5);

@@ -180,6 +180,21 @@ def test_allpairs_host_call(clusco, c1):
     assert torch.equal(out, ref)
 
 
+def test_allpairs_host_call_chunked_and_pool_release(clusco):
+    """Large enough (> 8 MB of results) to take the 8-chunk pipelined path; pinned and pageable host memory;
+    the result is bit-identical to the device-pointer call, before and after the pool is released."""
+    import torch
+    ens = wl.make_config("C2")
+    ref = clusco.clusco_crmsd_allpairs(_dev(ens.coords)).cpu()
+    h_in = torch.from_numpy(ens.coords)
+    for pin in (True, False, True):
+        x = h_in.pin_memory() if pin else h_in
+        out = torch.empty(ref.numel(), dtype=torch.float32, pin_memory=pin)
+        clusco.clusco_crmsd_allpairs_host(x, out)
+        assert torch.equal(out, ref)
+        clusco.clusco_host_release()
+
+
 # ---- a6 one-vs-all --------------------------------------------------------------------------------------
 
 def test_one_vs_all_prefix(clusco):
