@@ -261,10 +261,8 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             }
             --rem;
             const uint32_t buf = n & 1;
-#if !(defined(I8_EXPERIMENT) && I8_EXPERIMENT >= 5)
             ptx::mbar_wait(ACC_EMPTY(buf), ((n >> 1) & 1) ^ 1);
             ptx::mbar_wait(B_FULL(stage), phase);
-#endif
             ptx::tc_fence_after();
             if (ptx::elect_one()) {
                 const uint32_t d = tmem + buf * I8_ACC_COLS;
@@ -288,9 +286,6 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         }
     } else {
         // ===== epilogue =====
-#if defined(I8_EXPERIMENT) && I8_EXPERIMENT == 6
-        if (true) goto done;
-#endif
         const int ew = warp - 2;
         const int team = ew >> 3, half = (ew & 7) >> 2;          // column half: models 8*half .. 8*half+7 of the tile
         const int quad = warp & 3;                               // TMEM lanes 32 quad .. 32 quad + 31
@@ -313,9 +308,13 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         } pend = {};
         bool have_pend = false;
         auto finish_pending = [&]() {
+#if defined(I8_EXPERIMENT) && (I8_EXPERIMENT == 1 || I8_EXPERIMENT >= 3)   // developer switch: no eq. 2 arithmetic
+            const float2 c = make_float2(pend.inv.c2.x + pend.inv.c1.x + pend.Thi, pend.inv.c2.y + pend.inv.d.y + pend.Thj.y);
+#else
             const float2 c = eq2_finish(eq2_energy(pend.inv), make_float2(pend.Thi, pend.Thi),
                                         make_float2(pend.Tlo, pend.Tlo), make_float2(pend.pw, pend.pw), pend.Thj,
                                         pend.Tlj, pend.pwj, P.invLk);
+#endif
             if (pend.ok0) pend.dst[0] = c.x;
             if (pend.ok1) pend.dst[4] = c.y;
         };
@@ -406,9 +405,6 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         }
         if (have_pend) finish_pending();
     }
-#if defined(I8_EXPERIMENT) && I8_EXPERIMENT == 6
-done:
-#endif
     ptx::tc_fence_before();
     __syncthreads();
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
