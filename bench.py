@@ -343,7 +343,9 @@ def one_vs_all_side(clusco, wl, pk, flush):
 
 
 def launches_per_step(engine):
-    return 3     # model_stats_kernel, operand-plane kernel, fused Gram+epilogue kernel
+    # i8tc: i8_prep_kernel (centring + R^2 + operand images) and gram_i8tc_kernel (Gram + eq. 2 + packed store);
+    # ffma: model_stats_kernel, ffma_plane_kernel, gram_ffma_kernel
+    return 2 if engine == 2 else 3
 
 
 if __name__ == "__main__":

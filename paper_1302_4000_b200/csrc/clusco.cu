@@ -122,18 +122,16 @@ int clusco_allpairs_prepare(const float* coords, int64_t N, int32_t L, void* wor
     if (st != CLUSCO_OK) return st;
     cudaStream_t s = (cudaStream_t)stream;
     char* ws = (char*)workspace;
+    if (engine == CLUSCO_ENGINE_I8TC) return i8tc_prepare(coords, N, L, w, ws, s);   // a1 + a2 + operand planes, one launch
     ModelStat* stats = (ModelStat*)(ws + w.off_stats);
     // a1 + a2: centroid, scale exponent, sum of squares per model
     model_stats_kernel<<<(unsigned)((w.Np + 7) / 8), 256, 0, s>>>(coords, N, w.Np, L, stats);
     CLUSCO_CUDA_TRY(cudaGetLastError());
-    if (engine == CLUSCO_ENGINE_FFMA) {
-        float* Yt = (float*)(ws + w.off_ffma);
-        dim3 g((unsigned)(w.Np / 32), (unsigned)((w.Lp16 + 63) / 64));
-        ffma_plane_kernel<<<g, 256, 0, s>>>(coords, N, w.Np, L, w.Lp16, stats, Yt);
-        CLUSCO_CUDA_TRY(cudaGetLastError());
-        return CLUSCO_OK;
-    }
-    return i8tc_prepare(coords, N, L, w, ws, stats, s);
+    float* Yt = (float*)(ws + w.off_ffma);
+    dim3 g((unsigned)(w.Np / 32), (unsigned)((w.Lp16 + 63) / 64));
+    ffma_plane_kernel<<<g, 256, 0, s>>>(coords, N, w.Np, L, w.Lp16, stats, Yt);
+    CLUSCO_CUDA_TRY(cudaGetLastError());
+    return CLUSCO_OK;
 }
 
 int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out_rows,

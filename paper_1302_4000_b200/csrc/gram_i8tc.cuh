@@ -26,6 +26,7 @@
 #pragma once
 #include "common.cuh"
 #include "epilogue.cuh"
+#include "prep.cuh"
 #include "tc_ptx.cuh"
 
 namespace clusco {
@@ -40,32 +41,70 @@ constexpr int I8_THREADS = (2 + I8_EPI_WARPS) * 32;
 
 static inline bool i8tc_supported(int32_t L) { return L >= 1 && L <= 32 * I8_MAX_KSTEPS; }
 
-// ---- operand planes ---------------------------------------------------------------------------------------
+// ---- a1 + a2 + operand planes, one launch --------------------------------------------------------------------
 // Ap[row_tile][digit][kstep][I8_A_SLAB], Bp[col_tile][kstep][I8_B_SLAB]; a slab is a grid of 8-row x 16-byte core
 // matrices: byte (row, k) of a slab sits at (row/8)*256 + (k/16)*128 + (row%8)*16 + k%16.
-// One warp per model slot; lane = atom within the k-step.
-__global__ void __launch_bounds__(256) i8_plane_kernel(const float* __restrict__ coords, int64_t N, int32_t L,
-                                                       int32_t ks, int64_t row_slots, int64_t col_slots,
-                                                       int64_t stat_slots, const ModelStat* __restrict__ stats,
-                                                       int8_t* __restrict__ Ap, int8_t* __restrict__ Bp,
-                                                       PairStat* __restrict__ pstat)
+// One warp per model slot.  The model is read ONCE, element-wise (coalesced), and stays in registers through
+// three passes: FP64 centroid -> max|a| (scale exponent) -> fixed-point integers I.  The integers of a round
+// (4 k-steps = 128 atoms) go through a warp-private shared-memory strip so that each lane can pack the digit
+// bytes of 4 consecutive atoms of one component into one 32-bit store of the operand images.
+constexpr int I8_PREP_WARPS = 8;
+constexpr int I8_PREP_STRIP = 4 * 97;          // ints per warp and round: 4 k-steps x (96 + 1 pad)
+
+__global__ void __launch_bounds__(I8_PREP_WARPS * 32) i8_prep_kernel(const float* __restrict__ coords, int64_t N, int32_t L,
+                                                                     int32_t ks, int64_t row_slots, int64_t col_slots,
+                                                                     int64_t stat_slots, int8_t* __restrict__ Ap,
+                                                                     int8_t* __restrict__ Bp, PairStat* __restrict__ pstat)
 {
-    const int lane = threadIdx.x & 31;
-    const int64_t n = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    __shared__ int strip_s[I8_PREP_WARPS][I8_PREP_STRIP];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int64_t n = (int64_t)blockIdx.x * I8_PREP_WARPS + wib;
     if (n >= stat_slots) return;
     const bool valid = n < N;
-    double mean[3] = {0.0, 0.0, 0.0};
-    double scale = 0.0;
-    int ex = 0;
-    bool finite_range = true;
-    if (valid) {
-        const ModelStat s = stats[n];
-        mean[0] = s.mean[0]; mean[1] = s.mean[1]; mean[2] = s.mean[2];
-        ex = max(-30, min(30, s.ex));
-        finite_range = s.ex <= 30;                         // coordinates beyond 2^30 Angstrom are not representable
-        scale = ldexp(I8_KAPPA, 23 - ex);
-    }
+    const int n_el = valid ? 3 * L : 0;
     const float* x = coords + n * (int64_t)L * 3;
+    // element e = 384 r + 32 t + lane of the model; its component is (2 t + lane) % 3  (384 and 30 t are multiples of 3)
+    const int l3 = lane % 3;
+    float v[2][12];
+    double acc[3] = {0.0, 0.0, 0.0};                       // acc[q]: component (q + l3) % 3, q = (2 t) % 3
+    bool finite = true;
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int t = 0; t < 12; ++t) {
+            const int e = 384 * r + 32 * t + lane;
+            const float xv = e < n_el ? x[e] : 0.0f;
+            v[r][t] = xv;
+            finite = finite && (fabsf(xv) <= 3.0e38f);
+            acc[(2 * t) % 3] += (double)xv;
+        }
+    // per-component sums: lane holds component c in acc[(c - l3 + 3) % 3]
+    double mean[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int q = (c - l3 + 3) % 3;
+        const double mine = q == 0 ? acc[0] : (q == 1 ? acc[1] : acc[2]);
+        mean[c] = warp_sum(mine) / (double)L;
+    }
+    double mq[3];                                          // centroid component matching acc[q]
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const int c = (q + l3) % 3;
+        mq[q] = c == 0 ? mean[0] : (c == 1 ? mean[1] : mean[2]);
+    }
+    float amax = 0.0f;
+#pragma unroll
+    for (int r = 0; r < 2; ++r)
+#pragma unroll
+        for (int t = 0; t < 12; ++t)
+            if (384 * r + 32 * t + lane < n_el) amax = fmaxf(amax, fabsf((float)((double)v[r][t] - mq[(2 * t) % 3])));
+    amax = warp_max(amax);
+    int ex = 0;
+    if (amax > 0.0f && amax < 3.0e38f) (void)frexpf(amax, &ex);          // amax = m 2^ex, m in [0.5, 1)
+    const bool finite_range = ex <= 30;                    // coordinates beyond 2^30 Angstrom are not representable
+    ex = max(-30, min(30, ex));
+    const double scale = valid ? ldexp(I8_KAPPA, 23 - ex) : 0.0;
+
     // A image: row tile n/32, quadrant w = (n%32)/8, row-in-group r = n%8, row group 4w + p
     const int64_t a_tile = n >> 5;
     const int a_w = (int)(n & 31) >> 3, a_r = (int)(n & 7);
@@ -73,42 +112,59 @@ __global__ void __launch_bounds__(256) i8_plane_kernel(const float* __restrict__
     const int64_t b_tile = n >> 4;
     const int m16 = (int)(n & 15);
     const int b_o = (m16 & 8) | ((m16 & 3) << 1) | ((m16 >> 2) & 1);
-    const int kc = lane >> 4, kb = lane & 15;
+    const int sub = lane >> 3, j = lane & 7;               // packing role: k-step 4 r + sub, atoms 4 j .. 4 j + 3 of it
+    const int kc = j >> 2, kb = (j & 3) * 4;
+    int* strip = strip_s[wib];
     unsigned long long sumsq = 0ull;
-    bool finite = true;
-    for (int kk = 0; kk < ks; ++kk) {
-        const int k = kk * 32 + lane;
 #pragma unroll
-        for (int p = 0; p < 3; ++p) {
+    for (int r = 0; r < 2; ++r) {
+        if (4 * r >= ks) break;                            // warp-uniform
+#pragma unroll
+        for (int t = 0; t < 12; ++t) {
+            const int el = 32 * t + lane;                  // element within the round
             int I = 0;
-            if (valid && k < L) {
-                const float xv = x[3 * k + p];
-                finite = finite && (fabsf(xv) <= 3.0e38f);
-                I = __double2int_rn(((double)xv - mean[p]) * scale);
-            }
+            if (384 * r + el < n_el) I = __double2int_rn(((double)v[r][t] - mq[(2 * t) % 3]) * scale);
             sumsq += (unsigned long long)((long long)I * (long long)I);
-            const int d2 = (int)(int8_t)(I & 0xff);
-            const int I1 = (I - d2) >> 8;
-            const int d1 = (int)(int8_t)(I1 & 0xff);
-            const int d0 = (I1 - d1) >> 8;
-            const int8_t dig[3] = {(int8_t)d0, (int8_t)d1, (int8_t)d2};
-            if (n < row_slots) {
+            strip[el + el / 96] = I;
+        }
+        __syncwarp();
+        const int kk = 4 * r + sub;
+        if (kk < ks) {
+#pragma unroll
+            for (int p = 0; p < 3; ++p) {
+                uint32_t w[3] = {0u, 0u, 0u};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int I = strip[97 * sub + 3 * (4 * j + i) + p];
+                    const int d2 = (int)(int8_t)(I & 0xff);
+                    const int I1 = (I - d2) >> 8;
+                    const int d1 = (int)(int8_t)(I1 & 0xff);
+                    const int d0 = (I1 - d1) >> 8;
+                    w[0] |= (uint32_t)(d0 & 0xff) << (8 * i);
+                    w[1] |= (uint32_t)(d1 & 0xff) << (8 * i);
+                    w[2] |= (uint32_t)(d2 & 0xff) << (8 * i);
+                }
+                if (n < row_slots) {
+#pragma unroll
+                    for (int a = 0; a < 3; ++a)
+                        *reinterpret_cast<uint32_t*>(Ap + ((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + p) * 256 +
+                                                     kc * 128 + a_r * 16 + kb) = w[a];
+                }
+                if (n < col_slots) {
+#pragma unroll
+                    for (int b = 0; b < 3; ++b)
+                        *reinterpret_cast<uint32_t*>(Bp + (b_tile * ks + kk) * I8_B_SLAB + b * 1536 +
+                                                     (2 * p + (b_o >> 3)) * 256 + kc * 128 + (b_o & 7) * 16 + kb) = w[b];
+                }
+            }
+            if (n < row_slots) {                           // the zero rows (p = 3) of this model's quadrant
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
-                    Ap[((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + p) * 256 + kc * 128 + a_r * 16 + kb] = dig[a];
-            }
-            if (n < col_slots) {
-#pragma unroll
-                for (int b = 0; b < 3; ++b)
-                    Bp[(b_tile * ks + kk) * I8_B_SLAB + b * 1536 + (2 * p + (b_o >> 3)) * 256 + kc * 128 + (b_o & 7) * 16 + kb] =
-                        dig[b];
+                    *reinterpret_cast<uint32_t*>(Ap + ((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + 3) * 256 +
+                                                 kc * 128 + a_r * 16 + kb) = 0u;
             }
         }
-        if (n < row_slots) {                               // the zero rows (p = 3) of this model's quadrant
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
-                Ap[((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + 3) * 256 + kc * 128 + a_r * 16 + kb] = 0;
-        }
+        __syncwarp();
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sumsq += __shfl_xor_sync(0xffffffffu, sumsq, o);
@@ -421,15 +477,14 @@ static inline int i8tc_stages(int ks)
     return st;
 }
 
-static inline int i8tc_prepare(const float* coords, int64_t N, int32_t L, const Workspace& w, char* ws,
-                               ModelStat* stats, cudaStream_t s)
+static inline int i8tc_prepare(const float* coords, int64_t N, int32_t L, const Workspace& w, char* ws, cudaStream_t s)
 {
     if (!i8tc_supported(L)) return CLUSCO_ERR_INVALID_ARG;
     const int ks = w.Lp32 / 32;
     const int64_t row_slots = w.row_tiles * I8_ROW_MODELS, col_slots = w.col_tiles * I8_COL_MODELS;
-    i8_plane_kernel<<<(unsigned)((w.Np + 7) / 8), 256, 0, s>>>(coords, N, L, ks, row_slots, col_slots, w.Np, stats,
-                                                               (int8_t*)(ws + w.off_i8a), (int8_t*)(ws + w.off_i8b),
-                                                               (PairStat*)(ws + w.off_pstat));
+    i8_prep_kernel<<<(unsigned)((w.Np + I8_PREP_WARPS - 1) / I8_PREP_WARPS), I8_PREP_WARPS * 32, 0, s>>>(
+        coords, N, L, ks, row_slots, col_slots, w.Np, (int8_t*)(ws + w.off_i8a), (int8_t*)(ws + w.off_i8b),
+        (PairStat*)(ws + w.off_pstat));
     CLUSCO_CUDA_TRY(cudaGetLastError());
     return CLUSCO_OK;
 }
