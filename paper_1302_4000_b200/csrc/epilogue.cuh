@@ -26,7 +26,6 @@ namespace clusco {
 __device__ __forceinline__ float rcp_fast(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float rsqrt_fast(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float sqrt_fast(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
-__device__ __forceinline__ float cos_fast(float x) { float y; asm("cos.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
 
 // ---- the arithmetic of the closed form, written once for V = float (one pair per thread) and V = float2 (two
 // pairs per thread, evaluated together on the packed FFMA2 / FMUL2 / FADD2 instructions of sm_100; operand
@@ -61,22 +60,25 @@ template <class F> __device__ __forceinline__ float2 zip3(float2 a, float2 b, fl
 template <class V> struct EPairT { V E0; V delta; };
 typedef EPairT<float> EPair;
 
-// acos on [-1, 1]: sqrt(1 - |x|) * P7(|x|)  (Abramowitz & Stegun 4.4.46, |error| <= 2e-8), reflected for x < 0
+// cos(acos(x) / 3) on [-1, 1] (Viete's angle trisection) without the angle: with s = sqrt((1 + x) / 2) the
+// function is analytic on the whole of [0, 1] (the square-root branch point at x = -1 is absorbed by s, and at
+// x = +1 it is even in the angle), so one MUFU square root and a degree-7 minimax polynomial in s give it to
+// 1.3e-7 in fp32 Horner arithmetic (fitted on Chebyshev nodes against the FP64 definition).  x outside [-1, 1]
+// (rounding) is clamped by the saturating FMA.
 template <class V>
-__device__ __forceinline__ V acos_fast(V x)
+__device__ __forceinline__ V cos_third_acos(V x)
 {
     using namespace lp;
-    const V ax = map(x, [](float t) { return fabsf(t); });
-    V p = splat<V>(-0.0012624911f);
-    p = fma(p, ax, splat<V>(0.0066700901f));
-    p = fma(p, ax, splat<V>(-0.0170881256f));
-    p = fma(p, ax, splat<V>(0.0308918810f));
-    p = fma(p, ax, splat<V>(-0.0501743046f));
-    p = fma(p, ax, splat<V>(0.0889789874f));
-    p = fma(p, ax, splat<V>(-0.2145988016f));
-    p = fma(p, ax, splat<V>(1.5707963050f));
-    const V r = mul(map(sub(splat<V>(1.0f), ax), [](float t) { return sqrt_fast(t); }), p);
-    return zip(x, r, [](float xx, float rr) { return xx < 0.0f ? 3.14159265358979f - rr : rr; });
+    const V sv = map(x, [](float t) { return sqrt_fast(__saturatef(fmaf(t, 0.5f, 0.5f))); });
+    V p = splat<V>(1.1504285912e-03f);
+    p = fma(p, sv, splat<V>(-6.1699481236e-03f));
+    p = fma(p, sv, splat<V>(1.6159486845e-02f));
+    p = fma(p, sv, splat<V>(-3.0313061318e-02f));
+    p = fma(p, sv, splat<V>(5.2869105217e-02f));
+    p = fma(p, sv, splat<V>(-1.1104323939e-01f));
+    p = fma(p, sv, splat<V>(5.7734722249e-01f));
+    p = fma(p, sv, splat<V>(5.0000002277e-01f));
+    return p;
 }
 
 // a*b - c*d with one rounding error of the result (Kahan): w = c*d rounded, e = exact error of w
@@ -143,10 +145,8 @@ __device__ __forceinline__ EPairT<V> eq2_energy(const EqInvariants<V> inv)
                      splat<V>(1.0f / 54.0f));
     const V sp = map(pp, [](float t) { return sqrt_fast(t); });
     const V ps = mul(pp, sp);
-    V ratio = zip3(pp, rr, ps, [](float p_, float r_, float ps_) { return p_ > 0.0f ? r_ * rcp_fast(ps_) : 1.0f; });
-    ratio = map(ratio, [](float t) { return fminf(1.0f, fmaxf(-1.0f, t)); });
-    const V theta = mul(acos_fast(ratio), splat<V>(1.0f / 3.0f));     // in [0, pi/3]
-    V l1 = fma(mul(splat<V>(2.0f), sp), map(theta, [](float t) { return cos_fast(t); }), q);
+    const V ratio = zip3(pp, rr, ps, [](float p_, float r_, float ps_) { return p_ > 0.0f ? r_ * rcp_fast(ps_) : 1.0f; });
+    V l1 = fma(mul(splat<V>(2.0f), sp), cos_third_acos(ratio), q);    // cos(theta / 3), theta = acos(ratio) in [0, pi]
     l1 = zip(l1, q, [](float a_, float b_) { return fmaxf(a_, b_); }); // l1 >= trace/3 always
     const V is1 = map(l1, [](float t) { return rsqrt_fast(t); });
     const V s1 = mul(l1, is1);

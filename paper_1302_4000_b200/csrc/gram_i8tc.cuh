@@ -346,9 +346,12 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         const int team = ew >> 3, half = (ew & 7) >> 2;          // column half: models 8*half .. 8*half+7 of the tile
         const int quad = warp & 3;                               // TMEM lanes 32 quad .. 32 quad + 31
         const int r = lane >> 2, c4 = lane & 3;
-        int64_t I = I0, J = J0;
-        if (team == 1 && ++J >= Tc) { ++I; J = 2 * I; }
-        int64_t curI = -1, i = 0, rowoff = 0;
+        // tile coordinates and model indices fit 32 bits (N <= 2^24); only the packed offset needs 64
+        const int32_t Tc32 = (int32_t)Tc, N32 = (int32_t)P.N;
+        int32_t I = (int32_t)I0, J = (int32_t)J0;
+        if (team == 1 && ++J >= Tc32) { ++I; J = 2 * I; }
+        int32_t curI = -1, i = 0;
+        int64_t rowoff = 0;
         bool row_ok = false;
         PairStat si = {0.0f, 0.0f, 1.0f, 0.0f};
         // The closed form of a tile is evaluated in two halves, software-pipelined over the team's tiles: the
@@ -378,12 +381,12 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             if (I != curI) {                                     // per-row quantities (warp-uniform branch)
                 curI = I;
                 i = I * I8_ROW_MODELS + quad * 8 + r;
-                row_ok = i < P.N && i >= P.row_begin && i < P.row_end;
+                row_ok = i < N32 && i >= (int32_t)P.row_begin && i < (int32_t)P.row_end;
                 si = P.pstat[i];                                 // slots beyond N hold neutral records
-                rowoff = i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
+                rowoff = (int64_t)i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
             }
             // per-model records of this thread's two column models, requested before the accumulator wait
-            const int64_t j0 = J * I8_COL_MODELS + half * 8 + c4;
+            const int32_t j0 = J * I8_COL_MODELS + half * 8 + c4;
             const PairStat sj0 = P.pstat[j0], sj1 = P.pstat[j0 + 4];
             const uint32_t buf = (uint32_t)team;                 // tile n uses accumulator n & 1 = team
             ptx::mbar_wait(ACC_FULL(buf), (n >> 1) & 1);
@@ -451,13 +454,13 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             pend.Tlj = make_float2(sj0.Tlo, sj1.Tlo);
             pend.pwj = make_float2(sj0.pw, sj1.pw);
             pend.dst = P.out + rowoff + j0;
-            pend.ok0 = row_ok && j0 < P.N && j0 > i;             // masked pairs are simply not stored
-            pend.ok1 = row_ok && j0 + 4 < P.N && j0 + 4 > i;
+            pend.ok0 = row_ok && j0 < N32 && j0 > i;             // masked pairs are simply not stored
+            pend.ok1 = row_ok && j0 + 4 < N32 && j0 + 4 > i;
             have_pend = true;
             // advance two tiles
 #pragma unroll
             for (int s = 0; s < 2; ++s)
-                if (++J >= Tc) { ++I; J = 2 * I; }
+                if (++J >= Tc32) { ++I; J = 2 * I; }
         }
         if (have_pend) finish_pending();
     }
