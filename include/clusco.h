@@ -109,6 +109,31 @@ int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row
                             void* workspace, size_t workspace_bytes, int engine, void* stream);
 
 /*
+ * Fused consumers of the all-versus-all matrix (the matrix itself is never written to memory).
+ *
+ * clusco_crmsd_allpairs_below -- the paper's first use case computes all-versus-all cRMSD and keeps the pairs
+ * below a cut-off ("awk '{if($3<3.2) ...}'").  Here the filter and the compaction run in the
+ * epilogue of the all-pairs kernel:  for every i < j with cRMSD(i,j) < cutoff (compared in fp32 on the value
+ * the all-pairs call would store) one triple pair_i[k] = i, pair_j[k] = j, pair_c[k] = cRMSD is written; the
+ * order of the triples is unspecified.  *count (device, 8 bytes) receives the number of such pairs; if it
+ * exceeds `capacity` the first `capacity` slots are valid and the rest were dropped (call again with more).
+ * NaN pairs are never below.  capacity == 0 counts only (the three arrays may then be NULL).
+ *
+ * clusco_crmsd_rowstats -- the per-model reductions that cluster-representative selection consumes (mean
+ * cRMSD of a model to the others, neighbour counts within a cut-off):
+ *     rowsum[i] = sum_{j != i} cRMSD(i,j)   (float64; summation order unspecified: atomics),
+ *     below[i]  = #{ j != i : cRMSD(i,j) < cutoff }.
+ * A NaN/Inf model makes its own rowsum and every other rowsum NaN (it is a term of each).
+ *
+ * workspace: as clusco_crmsd_allpairs.  Both calls are asynchronous on `stream`.
+ */
+int clusco_crmsd_allpairs_below(const float* coords, int64_t N, int32_t L, float cutoff, int64_t capacity,
+                                int32_t* pair_i, int32_t* pair_j, float* pair_c, unsigned long long* count,
+                                void* workspace, size_t workspace_bytes, void* stream);
+int clusco_crmsd_rowstats(const float* coords, int64_t N, int32_t L, float cutoff, double* rowsum,
+                          int32_t* below, void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * One reference structure against N models: native[L][3], coords[N][L][3]
  * (neither pre-centred) -> out[N], out[k] = cRMSD(native, model k).
  */

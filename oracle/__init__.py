@@ -174,3 +174,43 @@ def crmsd_one_vs_all(native, coords):
     c2 = np.empty(N, np.float64)
     _load().oracle_crmsd_one_vs_all(_p(nat, _f32p), _p(x, _f32p), N, L, _p(c, _f64p), _p(c2, _f64p))
     return c, c2
+
+
+# ---- consumers of the matrix, written out from their definitions -------------------
+def pairs_below(coords, cutoff):
+    """The paper's first use case: all-versus-all cRMSD, keep the pairs below a cut-off.
+    Returns (i, j, c) of every i < j with c(i,j) < cutoff, in row-major order, from the FP64 matrix."""
+    x = _f32(coords)
+    N = x.shape[0]
+    c, _ = crmsd_allpairs(x)
+    ii, jj, cc = [], [], []
+    k = 0
+    for i in range(N):                      # plain loops over the packed triangle, row by row
+        row = c[k:k + N - 1 - i]
+        hit = np.nonzero(row < cutoff)[0]
+        ii.extend([i] * hit.size)
+        jj.extend((hit + i + 1).tolist())
+        cc.extend(row[hit].tolist())
+        k += N - 1 - i
+    return np.asarray(ii, np.int64), np.asarray(jj, np.int64), np.asarray(cc, np.float64)
+
+
+def rowstats(coords, cutoff):
+    """Per-model reductions used by representative selection: rowsum[i] = sum_{j != i} c(i,j) and
+    below[i] = #{j != i : c(i,j) < cutoff}, both from the FP64 matrix (symmetric: c(i,j) = c(j,i))."""
+    x = _f32(coords)
+    N = x.shape[0]
+    c, _ = crmsd_allpairs(x)
+    rowsum = np.zeros(N, np.float64)
+    below = np.zeros(N, np.int64)
+    k = 0
+    for i in range(N):
+        for j in range(i + 1, N):
+            v = c[k]
+            rowsum[i] += v
+            rowsum[j] += v
+            if v < cutoff:
+                below[i] += 1
+                below[j] += 1
+            k += 1
+    return rowsum, below

@@ -25,7 +25,7 @@ EXPORTS = (
     "clusco_crmsd_allpairs_workspace", "clusco_crmsd_allpairs", "clusco_crmsd_allpairs_ex",
     "clusco_crmsd_one_vs_all", "clusco_crmsd_allpairs_host", "clusco_crmsd_one_vs_all_host",
     "clusco_partition_rows", "clusco_engine_supported", "clusco_allpairs_prepare", "clusco_allpairs_compute",
-    "clusco_host_release",
+    "clusco_host_release", "clusco_crmsd_allpairs_below", "clusco_crmsd_rowstats",
 )
 
 
@@ -66,6 +66,8 @@ def load(build_if_missing: bool = False):
     lib.clusco_engine_supported.argtypes = [ctypes.c_int, i32]
     lib.clusco_allpairs_prepare.argtypes = [vp, i64, i32, vp, sz, ctypes.c_int, vp]
     lib.clusco_allpairs_compute.argtypes = [i64, i32, i64, i64, vp, vp, sz, ctypes.c_int, vp]
+    lib.clusco_crmsd_allpairs_below.argtypes = [vp, i64, i32, ctypes.c_float, i64, vp, vp, vp, vp, vp, sz, vp]
+    lib.clusco_crmsd_rowstats.argtypes = [vp, i64, i32, ctypes.c_float, vp, vp, vp, sz, vp]
     for name in EXPORTS:                       # every declared symbol must be exported
         getattr(lib, name)
     _lib = lib
@@ -175,6 +177,42 @@ def clusco_allpairs_compute(N: int, L: int, out, workspace, engine: int = ENGINE
                                             _stream_ptr(out))
     _check(st, "clusco_allpairs_compute")
     return out
+
+
+def clusco_crmsd_allpairs_below(coords, cutoff: float, capacity: int, workspace=None):
+    """Pairs with cRMSD < cutoff, compacted: returns (pair_i int32[capacity], pair_j, pair_c float32, count int64[1]);
+    the first min(count, capacity) slots are valid, in unspecified order (include/clusco.h)."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    dev = coords.device
+    pi = torch.empty(capacity, dtype=torch.int32, device=dev)
+    pj = torch.empty(capacity, dtype=torch.int32, device=dev)
+    pc = torch.empty(capacity, dtype=torch.float32, device=dev)
+    count = torch.empty(1, dtype=torch.int64, device=dev)
+    if workspace is None:
+        workspace = torch.empty(clusco_crmsd_allpairs_workspace(N, L), dtype=torch.uint8, device=dev)
+    with torch.cuda.device(dev):
+        st = load().clusco_crmsd_allpairs_below(_ptr(coords), N, L, float(cutoff), capacity, _ptr(pi), _ptr(pj), _ptr(pc),
+                                                _ptr(count), _ptr(workspace),
+                                                workspace.numel() * workspace.element_size(), _stream_ptr(coords))
+    _check(st, "clusco_crmsd_allpairs_below")
+    return pi, pj, pc, count
+
+
+def clusco_crmsd_rowstats(coords, cutoff: float, workspace=None):
+    """Per-model reductions of the all-vs-all matrix: (rowsum float64[N], below int32[N]) (include/clusco.h)."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    dev = coords.device
+    rowsum = torch.empty(N, dtype=torch.float64, device=dev)
+    below = torch.empty(N, dtype=torch.int32, device=dev)
+    if workspace is None:
+        workspace = torch.empty(clusco_crmsd_allpairs_workspace(N, L), dtype=torch.uint8, device=dev)
+    with torch.cuda.device(dev):
+        st = load().clusco_crmsd_rowstats(_ptr(coords), N, L, float(cutoff), _ptr(rowsum), _ptr(below), _ptr(workspace),
+                                          workspace.numel() * workspace.element_size(), _stream_ptr(coords))
+    _check(st, "clusco_crmsd_rowstats")
+    return rowsum, below
 
 
 def clusco_crmsd_one_vs_all(native, coords, out=None):

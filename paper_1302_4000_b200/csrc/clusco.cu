@@ -134,8 +134,12 @@ int clusco_allpairs_prepare(const float* coords, int64_t N, int32_t L, void* wor
     return CLUSCO_OK;
 }
 
-int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out_rows,
-                            void* workspace, size_t workspace_bytes, int engine, void* stream)
+}  // extern "C"
+
+// steps a3-a5 for rows [row_begin, row_end) from a prepared workspace; MODE selects the epilogue's sink
+template <int MODE>
+static int allpairs_compute_mode(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out_rows, const Sink& sink,
+                                 void* workspace, size_t workspace_bytes, int engine, void* stream)
 {
     if (N < 0 || L < 1) return CLUSCO_ERR_INVALID_ARG;
     engine = resolve_engine(engine, L);
@@ -143,7 +147,7 @@ int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row
     if (N < 2) return (row_begin == 0 && row_end >= 0) ? CLUSCO_OK : CLUSCO_ERR_INVALID_ARG;
     if (row_begin < 0 || row_end < row_begin || row_end > N) return CLUSCO_ERR_INVALID_ARG;
     if (row_begin == row_end) return CLUSCO_OK;
-    if (row_begin % 128 != 0 || !out_rows) return CLUSCO_ERR_INVALID_ARG;
+    if (row_begin % 128 != 0 || (MODE == SINK_STORE && !out_rows)) return CLUSCO_ERR_INVALID_ARG;
     const Workspace w = workspace_layout(N, L);
     if (!workspace || workspace_bytes < w.total || ((uintptr_t)workspace & 255u)) return CLUSCO_ERR_WORKSPACE_TOO_SMALL;
     int sms = 0;
@@ -151,9 +155,9 @@ int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row
     if (st != CLUSCO_OK) return st;
     cudaStream_t s = (cudaStream_t)stream;
     char* ws = (char*)workspace;
-    ModelStat* stats = (ModelStat*)(ws + w.off_stats);
-    const float invL = 1.0f / (float)L;
     if (engine == CLUSCO_ENGINE_FFMA) {
+        const ModelStat* stats = (const ModelStat*)(ws + w.off_stats);
+        const float invL = 1.0f / (float)L;
         const float* Yt = (const float*)(ws + w.off_ffma);
         TileRange tr;
         tr.T = (N + FF_TILE - 1) / FF_TILE;
@@ -162,12 +166,73 @@ int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row
         const int64_t W = tr.T - tr.I_lo, R = tr.I_hi - tr.I_lo;
         const int64_t tiles = R * W - R * (R - 1) / 2;
         if (tiles > 0x7fffffff) return CLUSCO_ERR_INVALID_ARG;
-        gram_ffma_kernel<<<(unsigned)tiles, 256, 0, s>>>(Yt, stats, N, w.Np, w.Lp16, invL, tr, row_begin, row_end,
-                                                        out_rows);
+        gram_ffma_kernel<MODE><<<(unsigned)tiles, 256, 0, s>>>(Yt, stats, N, w.Np, w.Lp16, invL, tr, row_begin, row_end,
+                                                              out_rows, sink);
         CLUSCO_CUDA_TRY(cudaGetLastError());
         return CLUSCO_OK;
     }
-    return i8tc_compute(N, L, row_begin, row_end, out_rows, w, ws, stats, sms, s);
+    return i8tc_compute<MODE>(N, L, row_begin, row_end, out_rows, sink, w, ws, sms, s);
+}
+
+extern "C" {
+
+int clusco_allpairs_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out_rows,
+                            void* workspace, size_t workspace_bytes, int engine, void* stream)
+{
+    return allpairs_compute_mode<SINK_STORE>(N, L, row_begin, row_end, out_rows, Sink{}, workspace, workspace_bytes, engine,
+                                             stream);
+}
+
+// NEXT-1a: threshold filter + compaction fused into the epilogue
+int clusco_crmsd_allpairs_below(const float* coords, int64_t N, int32_t L, float cutoff, int64_t capacity,
+                                int32_t* pair_i, int32_t* pair_j, float* pair_c, unsigned long long* count,
+                                void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (N < 0 || L < 1 || capacity < 0 || !count) return CLUSCO_ERR_INVALID_ARG;
+    if (capacity > 0 && (!pair_i || !pair_j || !pair_c)) return CLUSCO_ERR_INVALID_ARG;
+    if (N >= 2) {                                               // validate before touching `count`
+        int st = clusco_allpairs_prepare(coords, N, L, workspace, workspace_bytes, CLUSCO_ENGINE_AUTO, stream);
+        if (st != CLUSCO_OK) return st;
+    } else {
+        int st = check_device(nullptr);
+        if (st != CLUSCO_OK) return st;
+    }
+    CLUSCO_CUDA_TRY(cudaMemsetAsync(count, 0, sizeof(unsigned long long), (cudaStream_t)stream));
+    if (N < 2) return CLUSCO_OK;
+    Sink sink{};
+    sink.cutoff = cutoff;
+    sink.capacity = capacity;
+    sink.pair_i = pair_i;
+    sink.pair_j = pair_j;
+    sink.pair_c = pair_c;
+    sink.count = count;
+    return allpairs_compute_mode<SINK_BELOW>(N, L, 0, N, nullptr, sink, workspace, workspace_bytes, CLUSCO_ENGINE_AUTO,
+                                             stream);
+}
+
+// NEXT-1b: per-model row sums and neighbour counts fused into the epilogue
+int clusco_crmsd_rowstats(const float* coords, int64_t N, int32_t L, float cutoff, double* rowsum, int32_t* below,
+                          void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (N < 0 || L < 1) return CLUSCO_ERR_INVALID_ARG;
+    if (N == 0) return CLUSCO_OK;
+    if (!rowsum || !below) return CLUSCO_ERR_INVALID_ARG;
+    if (N >= 2) {
+        int st = clusco_allpairs_prepare(coords, N, L, workspace, workspace_bytes, CLUSCO_ENGINE_AUTO, stream);
+        if (st != CLUSCO_OK) return st;
+    } else {
+        int st = check_device(nullptr);
+        if (st != CLUSCO_OK) return st;
+    }
+    CLUSCO_CUDA_TRY(cudaMemsetAsync(rowsum, 0, sizeof(double) * (size_t)N, (cudaStream_t)stream));
+    CLUSCO_CUDA_TRY(cudaMemsetAsync(below, 0, sizeof(int32_t) * (size_t)N, (cudaStream_t)stream));
+    if (N < 2) return CLUSCO_OK;
+    Sink sink{};
+    sink.cutoff = cutoff;
+    sink.rowsum = rowsum;
+    sink.below = below;
+    return allpairs_compute_mode<SINK_ROWSTATS>(N, L, 0, N, nullptr, sink, workspace, workspace_bytes, CLUSCO_ENGINE_AUTO,
+                                                stream);
 }
 
 int clusco_crmsd_allpairs_ex(const float* coords, int64_t N, int32_t L, int64_t row_begin, int64_t row_end,

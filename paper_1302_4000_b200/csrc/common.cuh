@@ -47,6 +47,47 @@ struct __align__(16) PairStat {
     float pad;
 };
 
+// ---- what the fused all-pairs kernels do with a finished pair (i < j, c = cRMSD) ---------------------------
+// STORE:    out[packed index]                                   (a5, the matrix itself)
+// BELOW:    compacted (i, j, c) triples of the pairs with c < cutoff -- the paper's first use case filters the
+//           full matrix for pairs below 3.2 A; the matrix is never written
+// ROWSTATS: rowsum[i] += c, rowsum[j] += c and the neighbour counts below[.] += (c < cutoff) -- the per-model
+//           reductions that representative selection consumes (mean cRMSD to the others)
+enum SinkMode { SINK_STORE = 0, SINK_BELOW = 1, SINK_ROWSTATS = 2 };
+struct Sink {
+    float cutoff;
+    int64_t capacity;               // BELOW: slots in pair_i / pair_j / pair_c
+    int32_t* pair_i;
+    int32_t* pair_j;
+    float* pair_c;
+    unsigned long long* count;      // BELOW: number of pairs found (may exceed capacity; extra pairs are dropped)
+    double* rowsum;                 // ROWSTATS
+    int32_t* below;
+};
+
+// one pair, no cooperation between threads (the CUDA-core engine and the ragged edges use this form)
+template <int MODE>
+__device__ __forceinline__ void sink_emit(const Sink& S, int32_t i, int32_t j, float c)
+{
+    if (MODE == SINK_BELOW) {
+        if (c < S.cutoff) {
+            const unsigned long long slot = atomicAdd(S.count, 1ull);
+            if ((int64_t)slot < S.capacity) {
+                S.pair_i[slot] = i;
+                S.pair_j[slot] = j;
+                S.pair_c[slot] = c;
+            }
+        }
+    } else if (MODE == SINK_ROWSTATS) {
+        atomicAdd(S.rowsum + i, (double)c);
+        atomicAdd(S.rowsum + j, (double)c);
+        if (c < S.cutoff) {
+            atomicAdd(S.below + i, 1);
+            atomicAdd(S.below + j, 1);
+        }
+    }
+}
+
 // ---- tensor-core engine geometry (gram_i8tc.cuh) ---------------------------------------------------
 constexpr int I8_ROW_MODELS = 32;      // models per row tile: 4 TMEM quadrants x 8 models; lane = r + 8 p (p = 3: zero rows)
 constexpr int I8_COL_MODELS = 16;      // models per column tile: MMA N = 3 x 16 = 48 per level block

@@ -45,10 +45,11 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
 
+template <int MODE>
 __global__ void __launch_bounds__(256, 2)
 gram_ffma_kernel(const float* __restrict__ Yt, const ModelStat* __restrict__ stats, int64_t N, int64_t Np,
                  int32_t Lp16, float invL, TileRange tr, int64_t row_begin, int64_t row_end,
-                 float* __restrict__ out)
+                 float* __restrict__ out, const Sink sink)
 {
     __shared__ __align__(16) float As[2][FF_KC][FF_LD];
     __shared__ __align__(16) float Bs[2][FF_KC][FF_LD];
@@ -131,7 +132,9 @@ gram_ffma_kernel(const float* __restrict__ Yt, const ModelStat* __restrict__ sta
             for (int p = 0; p < 3; ++p)
 #pragma unroll
                 for (int q = 0; q < 3; ++q) m[3 * p + q] = tot[6 * (3 * a + p) + 3 * b + q];
-            out[packed_index(i, j, N) - base] = eq2_crmsd(m, si.Shi, si.Slo, si.ex, sj.Shi, sj.Slo, sj.ex, invL);
+            const float c = eq2_crmsd(m, si.Shi, si.Slo, si.ex, sj.Shi, sj.Slo, sj.ex, invL);
+            if (MODE == SINK_STORE) out[packed_index(i, j, N) - base] = c;
+            else sink_emit<MODE>(sink, (int32_t)i, (int32_t)j, c);
         }
     }
 }

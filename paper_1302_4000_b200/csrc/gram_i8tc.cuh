@@ -211,12 +211,15 @@ struct I8Params {
     int32_t stages;        // B ring depth (one stage = the whole column tile, KS k-steps)
     float invLk;           // 1 / (KAPPA^2 L)
     I8Tiles tiles;
+    Sink sink;             // MODE != SINK_STORE: where finished pairs go instead of `out`
 };
 
 // KS = k-steps (32 atoms each) per model, a template parameter so that the 3 KS MMAs of a tile are issued as
 // straight-line code with immediate operand offsets: the issuing warp is the critical resource of this kernel
 // (3 MMAs of 72 + 48 + 24 tensor cycles per k-step leave ~48 cycles of issue time per MMA).
-template <int KS>
+// MODE (SinkMode) selects what the epilogue does with a finished pair: packed store (a5), threshold compaction or
+// per-model row statistics (the fused consumers of the matrix).
+template <int KS, int MODE>
 __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params P)
 {
     extern __shared__ __align__(128) uint8_t smem[];
@@ -363,9 +366,19 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             float Thi, Tlo, pw;                  // row model
             float2 Thj, Tlj, pwj;                // the two column models
             float* dst;                          // out + rowoff + j0
+            int32_t i, j0;                       // the pairs are (i, j0) and (i, j0 + 4)
             bool ok0, ok1;
         } pend = {};
         bool have_pend = false;
+        // ROWSTATS: running sum / count of the row this lane group is on (rows persist over consecutive tiles)
+        double acc_sum = 0.0;
+        int32_t acc_cnt = 0, acc_i = -1;
+        auto flush_row = [&]() {
+            if (c4 == 0 && acc_i >= 0 && acc_i < (int32_t)P.N) {
+                atomicAdd(P.sink.rowsum + acc_i, acc_sum);
+                if (acc_cnt) atomicAdd(P.sink.below + acc_i, acc_cnt);
+            }
+        };
         auto finish_pending = [&]() {
 #if defined(I8_EXPERIMENT) && (I8_EXPERIMENT == 1 || I8_EXPERIMENT >= 3)   // developer switch: no eq. 2 arithmetic
             const float2 c = make_float2(pend.inv.c2.x + pend.inv.c1.x + pend.Thi, pend.inv.c2.y + pend.inv.d.y + pend.Thj.y);
@@ -374,8 +387,49 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                                         make_float2(pend.Tlo, pend.Tlo), make_float2(pend.pw, pend.pw), pend.Thj,
                                         pend.Tlj, pend.pwj, P.invLk);
 #endif
-            if (pend.ok0) pend.dst[0] = c.x;
-            if (pend.ok1) pend.dst[4] = c.y;
+            if (MODE == SINK_STORE) {
+                if (pend.ok0) pend.dst[0] = c.x;
+                if (pend.ok1) pend.dst[4] = c.y;
+            } else if (MODE == SINK_BELOW) {
+                if (pend.ok0) sink_emit<SINK_BELOW>(P.sink, pend.i, pend.j0, c.x);
+                if (pend.ok1) sink_emit<SINK_BELOW>(P.sink, pend.i, pend.j0 + 4, c.y);
+            } else {
+                // the warp holds 8 rows (r) x 8 columns (c4, c4 + 4): reduce over the columns for the row sums
+                // (kept in registers until the row changes) and over the rows for the column sums
+                float cx = pend.ok0 ? c.x : 0.0f, cy = pend.ok1 ? c.y : 0.0f;
+                int32_t bc = (pend.ok0 && c.x < P.sink.cutoff ? 1 : 0) | (pend.ok1 && c.y < P.sink.cutoff ? 1 << 16 : 0);
+                float rs = cx + cy;
+                int32_t rb = (bc & 0xffff) + (bc >> 16);
+#pragma unroll
+                for (int o = 1; o <= 2; o <<= 1) {
+                    rs += __shfl_xor_sync(0xffffffffu, rs, o);
+                    rb += __shfl_xor_sync(0xffffffffu, rb, o);
+                }
+                if (pend.i != acc_i) {
+                    flush_row();
+                    acc_i = pend.i;
+                    acc_sum = 0.0;
+                    acc_cnt = 0;
+                }
+                acc_sum += (double)rs;
+                acc_cnt += rb;
+#pragma unroll
+                for (int o = 4; o <= 16; o <<= 1) {
+                    cx += __shfl_xor_sync(0xffffffffu, cx, o);
+                    cy += __shfl_xor_sync(0xffffffffu, cy, o);
+                    bc += __shfl_xor_sync(0xffffffffu, bc, o);
+                }
+                if (r == 0) {
+                    if (pend.j0 < (int32_t)P.N) {
+                        atomicAdd(P.sink.rowsum + pend.j0, (double)cx);
+                        if (bc & 0xffff) atomicAdd(P.sink.below + pend.j0, bc & 0xffff);
+                    }
+                    if (pend.j0 + 4 < (int32_t)P.N) {
+                        atomicAdd(P.sink.rowsum + pend.j0 + 4, (double)cy);
+                        if (bc >> 16) atomicAdd(P.sink.below + pend.j0 + 4, bc >> 16);
+                    }
+                }
+            }
         };
         for (uint32_t n = team; n < ntiles; n += 2) {
             if (I != curI) {                                     // per-row quantities (warp-uniform branch)
@@ -454,6 +508,8 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             pend.Tlj = make_float2(sj0.Tlo, sj1.Tlo);
             pend.pwj = make_float2(sj0.pw, sj1.pw);
             pend.dst = P.out + rowoff + j0;
+            pend.i = i;
+            pend.j0 = j0;
             pend.ok0 = row_ok && j0 < N32 && j0 > i;             // masked pairs are simply not stored
             pend.ok1 = row_ok && j0 + 4 < N32 && j0 + 4 > i;
             have_pend = true;
@@ -463,6 +519,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 if (++J >= Tc32) { ++I; J = 2 * I; }
         }
         if (have_pend) finish_pending();
+        if (MODE == SINK_ROWSTATS) flush_row();
     }
     ptx::tc_fence_before();
     __syncthreads();
@@ -492,8 +549,9 @@ static inline int i8tc_prepare(const float* coords, int64_t N, int32_t L, const 
     return CLUSCO_OK;
 }
 
-static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out,
-                               const Workspace& w, char* ws, ModelStat*, int sms, cudaStream_t s)
+template <int MODE>
+static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t row_end, float* out, const Sink& sink,
+                               const Workspace& w, char* ws, int sms, cudaStream_t s)
 {
     if (!i8tc_supported(L)) return CLUSCO_ERR_INVALID_ARG;
     I8Params P;
@@ -501,6 +559,7 @@ static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t 
     P.Bp = (const int8_t*)(ws + w.off_i8b);
     P.pstat = (const PairStat*)(ws + w.off_pstat);
     P.out = out;
+    P.sink = sink;
     P.N = N;
     P.row_begin = row_begin;
     P.row_end = row_end;
@@ -518,8 +577,9 @@ static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t 
     switch (ks) {
 #define I8_LAUNCH(KS)                                                                                                  \
     case KS:                                                                                                           \
-        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gram_i8tc_kernel<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); \
-        gram_i8tc_kernel<KS><<<(unsigned)grid, I8_THREADS, smem, s>>>(P);                                              \
+        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gram_i8tc_kernel<KS, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize,  \
+                                             (int)smem));                                                              \
+        gram_i8tc_kernel<KS, MODE><<<(unsigned)grid, I8_THREADS, smem, s>>>(P);                                        \
         break;
         I8_LAUNCH(1) I8_LAUNCH(2) I8_LAUNCH(3) I8_LAUNCH(4) I8_LAUNCH(5) I8_LAUNCH(6) I8_LAUNCH(7) I8_LAUNCH(8)
 #undef I8_LAUNCH

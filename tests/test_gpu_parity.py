@@ -242,3 +242,97 @@ def test_one_vs_all_full_size_sampled(clusco):
         assert_parity(got, c_ref, c2_ref, f"C5 full size chunk {k}")
     out_h = clusco.clusco_crmsd_one_vs_all_host(torch.from_numpy(ens0.native), torch.from_numpy(keep[0][:5000]))
     assert torch.equal(out_h, out[:5000].cpu())
+
+
+# ---- NEXT-1: fused consumers of the matrix (threshold compaction, row statistics) ------------------------
+# Where fp32 decides an integer (c < cutoff) the GPU decides on its own fp32 value; the oracle's FP64 decision
+# may differ only for pairs within the cRMSD tolerance of the cut-off, so the checks bracket: everything the
+# oracle puts below cutoff - DELTA must be found, nothing at or above cutoff + DELTA may be.
+DELTA = 1.5e-3
+
+
+def _consumer_cases():
+    rng = np.random.default_rng(99)
+    long_chain = (rng.normal(size=(150, 300, 3)) * 8 + rng.uniform(-40, 40, size=(150, 1, 3))).astype(np.float32)
+    return [("C1", wl.make_config("C1").coords, 3.2), ("C2[:1000]", wl.make_config("C2", N=1000).coords, 6.0),
+            ("C3[:700]", wl.make_config("C3", N=700).coords, 3.2), ("L300-ffma", long_chain, 18.5)]
+
+
+@pytest.mark.parametrize("case", range(4))
+def test_pairs_below_matches_oracle(clusco, case):
+    name, x, cutoff = _consumer_cases()[case]
+    N = x.shape[0]
+    c_ref, c2_ref = oracle.crmsd_allpairs(x)
+    must = set(np.nonzero(c_ref < cutoff - DELTA)[0].tolist())
+    may = set(np.nonzero(c_ref < cutoff + DELTA)[0].tolist())
+    assert len(must) > 0, name
+    cap = len(may) + 16
+    pi, pj, pc, count = clusco.clusco_crmsd_allpairs_below(_dev(x), cutoff, cap)
+    n = int(count.item())
+    assert len(must) <= n <= len(may), (name, n, len(must), len(may))
+    pi, pj, pc = pi[:n].cpu().numpy().astype(np.int64), pj[:n].cpu().numpy().astype(np.int64), pc[:n].cpu().numpy()
+    assert np.all((0 <= pi) & (pi < pj) & (pj < N))
+    idx = wl.packed_index(pi, pj, N)
+    assert np.unique(idx).size == n, f"{name}: duplicate triples"
+    got = set(idx.tolist())
+    assert must <= got <= may, (name, len(must - got), len(got - may))
+    assert np.all(pc < cutoff)
+    assert_parity(pc, c_ref[idx], c2_ref[idx], f"{name} below")
+    # capacity overflow: the count is still the true number, and the filled slots are valid pairs
+    small = max(1, n // 3)
+    qi, qj, qc, count2 = clusco.clusco_crmsd_allpairs_below(_dev(x), cutoff, small)
+    assert int(count2.item()) == n
+    k2 = wl.packed_index(qi.cpu().numpy().astype(np.int64), qj.cpu().numpy().astype(np.int64), N)
+    assert set(k2.tolist()) <= got and np.unique(k2).size == small
+    # count-only call
+    _, _, _, count3 = clusco.clusco_crmsd_allpairs_below(_dev(x), cutoff, 0)
+    assert int(count3.item()) == n
+
+
+@pytest.mark.parametrize("case", range(4))
+def test_rowstats_match_oracle(clusco, case):
+    name, x, cutoff = _consumer_cases()[case]
+    N = x.shape[0]
+    rs_ref, _ = oracle.rowstats(x, cutoff)
+    _, lo = oracle.rowstats(x, cutoff - DELTA)
+    _, hi = oracle.rowstats(x, cutoff + DELTA)
+    rs, bl = clusco.clusco_crmsd_rowstats(_dev(x), cutoff)
+    rs, bl = rs.cpu().numpy(), bl.cpu().numpy().astype(np.int64)
+    # every term is within 1e-3 A of the oracle's (c >= 0.5 A); observed errors are far smaller, so ask for a
+    # mean per-term error below 2e-4 A, plus 0.05 A for the near-zero rigid-copy pair of C1 (tolerance on c^2 only)
+    assert np.abs(rs - rs_ref).max() <= 2e-4 * (N - 1) + 0.05, (name, np.abs(rs - rs_ref).max())
+    assert np.all(lo <= bl) and np.all(bl <= hi), name
+    assert bl.sum() % 2 == 0 and bl.sum() > 0
+
+
+def test_consumers_full_size_sampled(clusco):
+    """C3 at full size (the configuration bench.py times): sampled rows one by one against the oracle."""
+    ens = wl.make_config("C3")
+    N, cutoff = ens.N, 3.2
+    x = _dev(ens.coords)
+    rs, bl = clusco.clusco_crmsd_rowstats(x, cutoff)
+    rs, bl = rs.cpu().numpy(), bl.cpu().numpy()
+    pi, pj, pc, count = clusco.clusco_crmsd_allpairs_below(x, cutoff, 0)
+    assert int(count.item()) * 2 == int(bl.sum())                   # the two consumers agree on the fp32 decisions
+    for i in (0, 31, 4999, 9999):
+        others = np.array([j for j in range(N) if j != i], np.int64)
+        c_ref, _ = oracle.crmsd_pairs(ens.coords, np.minimum(i, others), np.maximum(i, others))
+        assert abs(rs[i] - c_ref.sum()) <= 2e-4 * (N - 1), (i, rs[i], c_ref.sum())
+        assert (c_ref < cutoff - DELTA).sum() <= bl[i] <= (c_ref < cutoff + DELTA).sum()
+
+
+def test_consumers_edge_cases(clusco):
+    import torch
+    x = _dev(wl.make_config("C1").coords)
+    for n in (0, 1):
+        pi, pj, pc, count = clusco.clusco_crmsd_allpairs_below(x[:n].contiguous(), 3.0, 4)
+        assert int(count.item()) == 0
+    rs, bl = clusco.clusco_crmsd_rowstats(x[:1].contiguous(), 3.0)
+    assert float(rs[0]) == 0.0 and int(bl[0]) == 0
+    # a NaN model is never "below" and poisons the row sums it is a term of
+    y = x[:64].clone()
+    y[5, 3, 1] = float("nan")
+    rs, bl = clusco.clusco_crmsd_rowstats(y, 1e9)
+    assert torch.isnan(rs).all() and int(bl[5]) == 0 and int(bl[0]) == 62
+    pi, pj, pc, count = clusco.clusco_crmsd_allpairs_below(y, 1e9, 64 * 63 // 2)
+    assert int(count.item()) == 63 * 62 // 2

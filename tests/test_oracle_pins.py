@@ -307,3 +307,28 @@ def test_P15_quartic_identity(c1):
         fp = 4 * E * (E * E - c2c) - 8 * det
         s3 = S * s[2]
         assert abs(fp - 8 * (s[0] + s[1]) * (s[0] + s3) * (s[1] + s3)) < 1e-9 * abs(E) ** 3
+
+
+def test_consumers_match_scipy_squareform(c1):
+    """pairs_below / rowstats against an independent unpacking of the packed triangle (scipy's condensed order)
+    and a closed form: for an ensemble of copies of ONE rigid body every c is ~0, so below = N-1 and rowsum ~ 0."""
+    from scipy.spatial.distance import squareform
+    x = c1.coords[:60]
+    c, _ = oracle.crmsd_allpairs(x)
+    D = squareform(c)                                   # full symmetric matrix, zero diagonal
+    cutoff = float(np.median(c))
+    rs, bl = oracle.rowstats(x, cutoff)
+    assert np.allclose(rs, D.sum(axis=1), rtol=0, atol=1e-9)
+    assert np.array_equal(bl, (D < cutoff).sum(axis=1) - 1)          # minus the diagonal zero
+    i, j, cc = oracle.pairs_below(x, cutoff)
+    iu, ju = np.nonzero(np.triu(D < cutoff, 1))
+    assert np.array_equal(i, iu) and np.array_equal(j, ju) and np.allclose(cc, D[iu, ju], rtol=0, atol=0)
+    assert i.size == (c < cutoff).sum() and 0 < i.size < c.size
+    # closed form: rigid copies of one structure
+    rng = np.random.default_rng(5)
+    base = rng.normal(size=(20, 3)) * 5
+    copies = np.stack([_rigid(base, rng) for _ in range(7)]).astype(np.float32)
+    rs, bl = oracle.rowstats(copies, 1e-3)
+    assert np.all(bl == 6) and np.all(rs < 1e-3)
+    i, j, cc = oracle.pairs_below(copies, 1e-3)
+    assert i.size == 21
