@@ -276,6 +276,9 @@ def main():
     ova = None
     if not args.no_ova and world == 1:
         ova = one_vs_all_side(clusco, wl, pk, flush)
+    consumers = None
+    if not args.no_ova and world == 1:
+        consumers = consumers_side(clusco, coords, ws, flush, P, ms_per_step)
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -291,7 +294,7 @@ def main():
                    "engine": {1: "ffma", 2: "i8tc"}[engine], "l2": "flushed between timed iterations (256 MB write)",
                    "effective_tflops": flops * world / (ms_per_step * 1e-3) / 1e12},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step(engine) * args.steps,
-        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova,
+        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova, "consumers": consumers,
     }))
     if dist:
         dist.destroy_process_group()
@@ -340,6 +343,32 @@ def one_vs_all_side(clusco, wl, pk, flush):
             "roofline": {"bound": "hbm", "achieved": gbs, "peak": pk["hbm_gbs"], "unit": "GB/s",
                          "frac": gbs / pk["hbm_gbs"], "traffic": _ncu_traffic("one_vs_all_stream_kernel", "C5"),
                          "algorithmic_bytes": nbytes, "kernel": "one_vs_all_stream_kernel"}}
+
+
+def consumers_side(clusco, coords, ws, flush, P, store_ms):
+    """NEXT-1: the same pass with the matrix consumed in the epilogue instead of stored --
+    pairs below 3.2 A (the paper's cut-off) compacted, and per-model row sums / neighbour counts."""
+    import torch
+    stream = torch.cuda.current_stream()
+    res = {}
+    for name, call in (("below_3.2A", lambda: clusco.clusco_crmsd_allpairs_below(coords, 3.2, 1 << 22, workspace=ws)),
+                       ("rowstats_3.2A", lambda: clusco.clusco_crmsd_rowstats(coords, 3.2, workspace=ws))):
+        for _ in range(3):
+            r = call()
+        reps = 10
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        torch.cuda.synchronize()
+        for a, b in ev:
+            flush.zero_()
+            a.record(stream)
+            r = call()
+            b.record(stream)
+        torch.cuda.synchronize()
+        ms = sum(a.elapsed_time(b) for a, b in ev) / reps
+        res[name] = {"ms": ms, "pairs_per_s": P / (ms * 1e-3), "vs_store_step": ms / store_ms}
+        if name.startswith("below"):
+            res[name]["pairs_found"] = int(r[3].item())
+    return res
 
 
 def launches_per_step(engine):
