@@ -26,14 +26,23 @@ _f64p = ctypes.POINTER(ctypes.c_double)
 _i64p = ctypes.POINTER(ctypes.c_int64)
 
 
+_SRC_D = os.path.join(_HERE, "drmsd_oracle.c")
+_LIB_D = os.path.join(_HERE, "libdrmsd_oracle.so")
+_lib_d = None
+
+
+def _compile(src: str, lib: str, force: bool) -> str:
+    if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
+        tmp = lib + f".tmp{os.getpid()}"
+        subprocess.run(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, src, "-lm"], check=True)
+        os.replace(tmp, lib)
+    return lib
+
+
 def build(force: bool = False) -> str:
-    """Compile crmsd_oracle.c -> libcrmsd_oracle.so (gcc -O2 -fopenmp, no fast-math)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
-        tmp = _LIB + f".tmp{os.getpid()}"
-        subprocess.run(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"],
-                       check=True)
-        os.replace(tmp, _LIB)
-    return _LIB
+    """Compile crmsd_oracle.c and drmsd_oracle.c (gcc -O2 -fopenmp, no fast-math); returns the cRMSD library."""
+    _compile(_SRC_D, _LIB_D, force)
+    return _compile(_SRC, _LIB, force)
 
 
 def _load():
@@ -214,3 +223,57 @@ def rowstats(coords, cutoff):
                 below[j] += 1
             k += 1
     return rowsum, below
+
+
+# ---- dRMSD (oracle = eq. 5 literally, drmsd_oracle.c) ------------------------------
+def _load_d():
+    global _lib_d
+    if _lib_d is None:
+        lib = ctypes.CDLL(_compile(_SRC_D, _LIB_D, False))
+        lib.oracle_drmsd_pair.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p]
+        lib.oracle_drmsd_pair.restype = ctypes.c_double
+        lib.oracle_drmsd_rows.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_int64, ctypes.c_int64,
+                                          _f64p, _f64p]
+        lib.oracle_drmsd_rows.restype = None
+        lib.oracle_drmsd_pairs.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, _i64p, _i64p, ctypes.c_int64,
+                                           _f64p, _f64p]
+        lib.oracle_drmsd_pairs.restype = None
+        _lib_d = lib
+    return _lib_d
+
+
+def drmsd_pair(xa, xb):
+    """eq. 5 for one pair: (d, d2)."""
+    a, b = _f32(xa), _f32(xb)
+    assert a.shape == b.shape
+    d2 = ctypes.c_double()
+    d = _load_d().oracle_drmsd_pair(_p(a, _f32p), _p(b, _f32p), a.shape[0], ctypes.byref(d2))
+    return float(d), float(d2.value)
+
+
+def drmsd_rows(coords, row_begin, row_end):
+    """Rows [row_begin,row_end) of the packed all-vs-all dRMSD matrix: (d, d2) fp64, row-major, j>i."""
+    x = _f32(coords)
+    N, L, _ = x.shape
+    n = (row_begin * (2 * N - row_begin - 1) // 2, row_end * (2 * N - row_end - 1) // 2)
+    d = np.empty(n[1] - n[0], np.float64)
+    d2 = np.empty(n[1] - n[0], np.float64)
+    _load_d().oracle_drmsd_rows(_p(x, _f32p), N, L, int(row_begin), int(row_end), _p(d, _f64p), _p(d2, _f64p))
+    return d, d2
+
+
+def drmsd_allpairs(coords):
+    x = _f32(coords)
+    return drmsd_rows(x, 0, x.shape[0])
+
+
+def drmsd_pairs(coords, pi, pj):
+    """Listed pairs: (d, d2)."""
+    x = _f32(coords)
+    N, L, _ = x.shape
+    pi = np.ascontiguousarray(pi, np.int64)
+    pj = np.ascontiguousarray(pj, np.int64)
+    d = np.empty(pi.size, np.float64)
+    d2 = np.empty(pi.size, np.float64)
+    _load_d().oracle_drmsd_pairs(_p(x, _f32p), N, L, _p(pi, _i64p), _p(pj, _i64p), pi.size, _p(d, _f64p), _p(d2, _f64p))
+    return d, d2

@@ -391,8 +391,31 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 if (pend.ok0) pend.dst[0] = c.x;
                 if (pend.ok1) pend.dst[4] = c.y;
             } else if (MODE == SINK_BELOW) {
-                if (pend.ok0) sink_emit<SINK_BELOW>(P.sink, pend.i, pend.j0, c.x);
-                if (pend.ok1) sink_emit<SINK_BELOW>(P.sink, pend.i, pend.j0 + 4, c.y);
+                // warp-aggregated append: one atomic on the shared counter per warp and tile
+                const bool h0 = pend.ok0 && c.x < P.sink.cutoff, h1 = pend.ok1 && c.y < P.sink.cutoff;
+                const uint32_t m0 = __ballot_sync(0xffffffffu, h0), m1 = __ballot_sync(0xffffffffu, h1);
+                if (m0 | m1) {
+                    unsigned long long base = 0ull;
+                    if (lane == 0) base = atomicAdd(P.sink.count, (unsigned long long)(__popc(m0) + __popc(m1)));
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    const uint32_t lt = (1u << lane) - 1u;
+                    if (h0) {
+                        const int64_t slot = (int64_t)base + __popc(m0 & lt);
+                        if (slot < P.sink.capacity) {
+                            P.sink.pair_i[slot] = pend.i;
+                            P.sink.pair_j[slot] = pend.j0;
+                            P.sink.pair_c[slot] = c.x;
+                        }
+                    }
+                    if (h1) {
+                        const int64_t slot = (int64_t)base + __popc(m0) + __popc(m1 & lt);
+                        if (slot < P.sink.capacity) {
+                            P.sink.pair_i[slot] = pend.i;
+                            P.sink.pair_j[slot] = pend.j0 + 4;
+                            P.sink.pair_c[slot] = c.y;
+                        }
+                    }
+                }
             } else {
                 // the warp holds 8 rows (r) x 8 columns (c4, c4 + 4): reduce over the columns for the row sums
                 // (kept in registers until the row changes) and over the rows for the column sums
