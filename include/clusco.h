@@ -134,6 +134,20 @@ int clusco_crmsd_rowstats(const float* coords, int64_t N, int32_t L, float cutof
                           int32_t* below, void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * All-versus-all distance RMSD, the paper's eq. 5:
+ *     dRMSD(A,B) = sqrt( 2/(L(L-1)) sum_{i<j} (d_ij^A - d_ij^B)^2 ),  d_ij = |x_i - x_j|
+ * (mirror images score 0: "loses chirality").  out[N(N-1)/2]: the same packed row-major upper
+ * triangle as clusco_crmsd_allpairs.  Computed as one tensor-core Gram contraction over the K = L(L-1)/2
+ * distances per model, in exact 3 x 8-bit fixed point; needs 2 <= L <= 296 (int32 accumulators), L = 1 gives
+ * all zeros, L > 296 -> CLUSCO_ERR_INVALID_ARG.  workspace: >= clusco_drmsd_allpairs_workspace(N, L) bytes
+ * (about 3 N K bytes: the int8 distance planes), 256-byte aligned.  NaN/Inf coordinates propagate to NaN
+ * for the pairs of that model.  Asynchronous on `stream`.
+ */
+size_t clusco_drmsd_allpairs_workspace(int64_t N, int32_t L);
+int clusco_drmsd_allpairs(const float* coords, int64_t N, int32_t L, float* out,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * One reference structure against N models: native[L][3], coords[N][L][3]
  * (neither pre-centred) -> out[N], out[k] = cRMSD(native, model k).
  */

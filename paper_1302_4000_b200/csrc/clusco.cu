@@ -8,6 +8,7 @@
 #include "common.cuh"
 #include "epilogue.cuh"
 #include "gram_ffma.cuh"
+#include "drmsd_i8tc.cuh"
 #include "gram_i8tc.cuh"
 #include "one_vs_all.cuh"
 #include "prep.cuh"
@@ -253,6 +254,34 @@ int clusco_crmsd_allpairs(const float* coords, int64_t N, int32_t L, float* out,
 {
     return clusco_crmsd_allpairs_ex(coords, N, L, 0, N < 0 ? 0 : N, out, workspace, workspace_bytes,
                                     CLUSCO_ENGINE_AUTO, stream);
+}
+
+// NEXT-2: all-versus-all dRMSD (eq. 5) as one tensor-core Gram over the distance vectors
+size_t clusco_drmsd_allpairs_workspace(int64_t N, int32_t L)
+{
+    if (N < 0 || L < 1 || L > DG_MAX_L) return 0;
+    if (N < 2 || L < 2) return 256;
+    return drmsd_workspace_layout(N, L).total;
+}
+
+int clusco_drmsd_allpairs(const float* coords, int64_t N, int32_t L, float* out, void* workspace, size_t workspace_bytes,
+                          void* stream)
+{
+    if (N < 0 || L < 1 || L > DG_MAX_L) return CLUSCO_ERR_INVALID_ARG;
+    if (N < 2) return CLUSCO_OK;
+    if (!coords || !out) return CLUSCO_ERR_INVALID_ARG;
+    if (N > (int64_t)1 << 24) return CLUSCO_ERR_INVALID_ARG;
+    int sms = 0;
+    int st = check_device(&sms);
+    if (st != CLUSCO_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (L < 2) {                                                // a single atom has no distance: every dRMSD is 0
+        CLUSCO_CUDA_TRY(cudaMemsetAsync(out, 0, sizeof(float) * (size_t)(N * (N - 1) / 2), s));
+        return CLUSCO_OK;
+    }
+    const DWorkspace w = drmsd_workspace_layout(N, L);
+    if (!workspace || workspace_bytes < w.total || ((uintptr_t)workspace & 255u)) return CLUSCO_ERR_WORKSPACE_TOO_SMALL;
+    return drmsd_launch(coords, N, L, out, (char*)workspace, sms, s);
 }
 
 // one launch, no scratch: every CTA centres the native into its own shared memory

@@ -1,0 +1,329 @@
+// drmsd_i8tc.cuh -- all-versus-all distance RMSD (the paper's eq. 5) as ONE Gram contraction on the
+// tensor cores.
+//
+// With d^A in R^K the vector of the K = L(L-1)/2 intra-model distances d_ij = |x_i - x_j| (i < j, row-major),
+//     dRMSD(A,B)^2 = (2 / (L(L-1))) sum_{i<j} (d_ij^A - d_ij^B)^2 = ( |d^A|^2 + |d^B|^2 - 2 d^A . d^B ) / K,
+// so the whole matrix is the N x K by K x N product D D^T plus a trivial epilogue.  The cancellation is as severe
+// as in eq. 2 of cRMSD (a difference of numbers ~K * R_g^2 that must be right to ~1e-3 A^2 * K), so the same exact
+// arithmetic is used: every model's distances are scaled by a power of two, multiplied by
+// KAPPA 2^23 and rounded to a 24-bit integer I = g0 2^16 + g1 2^8 + g2 (signed 8-bit digits); the dot product is
+//     sum_k I_A I_B = 2^32 V0 + 2^24 V1 + 2^16 V2 (+ two dropped low-order levels),
+// six int8 products accumulated EXACTLY in int32 TMEM accumulators (|V| <= 3 K 2^14 < 2^31 needs L <= 296), and
+// |d|^2 is taken from the same integers (exact in 64 bits), so quantisation cancels for similar models.
+//
+// Operand plane (one, shared by both operands): P[tile64][k-step][digit][2048 B] -- for 64 consecutive models and 32
+// consecutive entries of K, the int8 digit `digit` as a shared-memory image in tcgen05's canonical K-major no-swizzle
+// core-matrix layout (8 row groups x [2 x 128 B]), fetched by plain 1-D bulk copies.
+//
+// Kernel: persistent, one CTA per SM, tile = 128 x 128 models (two 64-column halves), warp 0 = bulk-copy producer
+// (ring of 24 KB stages: A = 3 digits x 128 rows, B = 2 halves x 3 digits x 64 rows), warp 1 = MMA issuer (six MMAs
+// per k-step: A(g0).[B(g0);B(g1);B(g2)]^T, A(g1).[B(g0);B(g1)]^T, A(g2).B(g0)^T for each half, N = 192/128/64),
+// warps 2..5 = epilogue (FP64: the K loop is ~1000 k-steps long, the epilogue is <1 % of a tile).
+#pragma once
+#include "common.cuh"
+#include "prep.cuh"
+#include "tc_ptx.cuh"
+
+namespace clusco {
+
+constexpr double DG_KAPPA = 127.0 / 128.0;
+constexpr int DG_MAX_L = 296;                  // 3 K 2^14 < 2^31 with K = L(L-1)/2
+constexpr int DG_TILE = 128, DG_HALF = 64;
+constexpr int DG_SLAB = 2048;                  // bytes of one (tile64, k-step, digit) image: 64 rows x 32 entries
+constexpr int DG_STAGE_BYTES = 3 * 2 * DG_SLAB + 2 * 3 * DG_SLAB;   // A (3 digits x 128 rows) + B (2 halves x 3 digits x 64)
+constexpr int DG_STAGES = 8;
+constexpr int DG_THREADS = 6 * 32;
+constexpr int DG_PREP_WARPS = 8;
+
+struct __align__(16) DStat {
+    double T;          // KAPPA^2 sum_k d_k^2 of the quantised distances, true scale (Angstrom^2); NaN poisons the model
+    float pw;          // 2^e, e = the model's scale exponent
+    float pad;
+};
+
+struct DWorkspace {
+    int64_t N, Np, K, ks, tiles64;
+    size_t off_stat, off_plane, total;
+};
+static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L)
+{
+    DWorkspace w;
+    w.N = N;
+    w.Np = round_up(N, DG_TILE);
+    w.K = (int64_t)L * (L - 1) / 2;
+    w.ks = (w.K + 31) / 32;
+    w.tiles64 = w.Np / DG_HALF;
+    size_t o = 0;
+    w.off_stat = o;
+    o += (size_t)round_up((int64_t)sizeof(DStat) * w.Np, 256);
+    w.off_plane = o;
+    o += (size_t)round_up(w.tiles64 * w.ks * 3 * DG_SLAB, 256);
+    w.total = o + 256;
+    return w;
+}
+
+// ---- distances, scale, digits, operand plane: one CTA per 8 consecutive models (one core-matrix row group), one
+// warp per model; lane = entry within the k-step.  Two passes over the K distances (max, then quantise), each
+// recomputed in FP64 from the fp32 coordinates held in shared memory.
+__global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const float* __restrict__ coords, int64_t N, int32_t L,
+                                                                        int64_t K, int64_t ks, int8_t* __restrict__ plane,
+                                                                        DStat* __restrict__ stat)
+{
+    __shared__ float xs[DG_PREP_WARPS][3 * DG_MAX_L];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t n = (int64_t)blockIdx.x * DG_PREP_WARPS + w;
+    const bool valid = n < N;
+    float* x = xs[w];
+    bool finite = true;
+    for (int e = lane; e < 3 * L; e += 32) {
+        const float v = valid ? coords[n * (int64_t)L * 3 + e] : 0.0f;
+        finite = finite && (fabsf(v) <= 3.0e38f);
+        x[e] = v;
+    }
+    __syncwarp();
+    auto dist2 = [&](int i, int j) {
+        const double dx = (double)x[3 * i] - (double)x[3 * j];
+        const double dy = (double)x[3 * i + 1] - (double)x[3 * j + 1];
+        const double dz = (double)x[3 * i + 2] - (double)x[3 * j + 2];
+        return dx * dx + dy * dy + dz * dz;
+    };
+    // pass 1: largest distance -> power-of-two scale with dmax 2^-ex in [0.5, 1)
+    double m2 = 0.0;
+    if (valid) {
+        int i = 0, pos = lane;                                   // entry k = lane, lane + 32, ...: pair (i, i + 1 + pos)
+        for (int64_t k = lane; k < K; k += 32) {
+            while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
+            m2 = fmax(m2, dist2(i, i + 1 + pos));
+            pos += 32;
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m2 = fmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
+    int ex = 0;
+    const double dmax = sqrt(m2);
+    if (dmax > 0.0 && dmax < 1.0e30) (void)frexp(dmax, &ex);
+    const bool in_range = dmax < 1.0e9;
+    ex = max(-30, min(30, ex));
+    const double scale = ldexp(DG_KAPPA, 23 - ex);
+    // pass 2: integers, digits, plane bytes
+    const int64_t t64 = n >> 6;
+    const int g = (int)(n & 63) >> 3, r8 = (int)(n & 7);
+    const int kc = lane >> 4, kb = lane & 15;
+    int8_t* base = plane + (t64 * ks * 3) * DG_SLAB + g * 256 + kc * 128 + r8 * 16 + kb;
+    long long sumsq = 0ll;
+    int i = 0, pos = lane;
+    for (int64_t kk = 0; kk < ks; ++kk) {
+        const int64_t k = kk * 32 + lane;
+        int I = 0;
+        if (valid && k < K) {
+            while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
+            I = __double2int_rn(sqrt(dist2(i, i + 1 + pos)) * scale);
+            pos += 32;
+        }
+        const int g2 = (int)(int8_t)(I & 0xff);
+        const int I1 = (I - g2) >> 8;
+        const int g1 = (int)(int8_t)(I1 & 0xff);
+        const int g0 = (I1 - g1) >> 8;
+        // |d|^2 from the SAME three levels the Gram keeps (I^2 minus the two dropped low-order levels), so that an
+        // identical pair cancels to exactly 0
+        sumsq += (long long)I * (long long)I - (long long)(512 * g1 * g2 + g2 * g2);
+        int8_t* p = base + kk * 3 * DG_SLAB;
+        p[0] = (int8_t)g0;
+        p[DG_SLAB] = (int8_t)g1;
+        p[2 * DG_SLAB] = (int8_t)g2;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) sumsq += __shfl_xor_sync(0xffffffffu, sumsq, o);
+    finite = __all_sync(0xffffffffu, finite);
+    if (lane == 0) {
+        DStat s;
+        s.T = ldexp((double)sumsq, 2 * ex - 46);
+        if (!finite || !in_range) s.T = __longlong_as_double(0x7ff8000000000000ll);
+        s.pw = pow2i(ex);
+        s.pad = 0.0f;
+        stat[n] = s;
+    }
+}
+
+// ---- the Gram kernel -------------------------------------------------------------------------------------------
+struct DGParams {
+    const int8_t* plane;
+    const DStat* stat;
+    float* out;
+    int64_t N, ks;
+    int32_t T;             // tiles per side (Np / 128); upper-triangle tiles I <= J are linearised row-major
+    int64_t total;         // T (T + 1) / 2
+    double invKk;          // 1 / (KAPPA^2 K)
+};
+
+__device__ __forceinline__ void dg_tile_from_linear(int64_t t, int32_t T, int32_t& I, int32_t& J)
+{
+    // rows before row I hold I T - I (I - 1) / 2 tiles
+    int32_t lo = 0, hi = T - 1;
+    while (lo < hi) {
+        const int32_t mid = (lo + hi + 1) >> 1;
+        if ((int64_t)mid * T - (int64_t)mid * (mid - 1) / 2 <= t) lo = mid; else hi = mid - 1;
+    }
+    I = lo;
+    J = I + (int32_t)(t - ((int64_t)I * T - (int64_t)I * (I - 1) / 2));
+}
+
+__global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParams P)
+{
+    extern __shared__ __align__(128) uint8_t smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)DG_STAGES * DG_STAGE_BYTES);
+    const uint32_t bar0 = ptx::smem_u32(bars);
+    auto FULL = [&](uint32_t s) { return bar0 + 8u * s; };
+    auto EMPTY = [&](uint32_t s) { return bar0 + 8u * (DG_STAGES + s); };
+    const uint32_t ACC_FULL = bar0 + 8u * (2 * DG_STAGES), ACC_EMPTY = ACC_FULL + 8u;
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * DG_STAGES + 2);
+
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < DG_STAGES; ++s) {
+            ptx::mbar_init(FULL(s), 1);
+            ptx::mbar_init(EMPTY(s), 1);
+        }
+        ptx::mbar_init(ACC_FULL, 1);
+        ptx::mbar_init(ACC_EMPTY, 4);
+        ptx::fence_mbar_init();
+    }
+    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
+    ptx::tc_fence_before();
+    __syncthreads();
+    ptx::tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    const int64_t ks = P.ks;
+
+    if (warp == 0) {
+        // ===== producer =====
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0;
+            for (int64_t t = blockIdx.x; t < P.total; t += gridDim.x) {
+                int32_t I, J;
+                dg_tile_from_linear(t, P.T, I, J);
+                const int8_t* a0 = P.plane + ((int64_t)(2 * I) * ks * 3) * DG_SLAB;       // tile64 2I; 2I + 1 follows at + ks * 3 slabs
+                const int8_t* b0 = P.plane + ((int64_t)(2 * J) * ks * 3) * DG_SLAB;
+                const int64_t t64_stride = ks * 3 * DG_SLAB;
+                for (int64_t kk = 0; kk < ks; ++kk) {
+                    ptx::mbar_wait(EMPTY(stage), phase ^ 1);
+                    ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
+                    const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
+                    const uint32_t sB = sA + 6 * DG_SLAB;
+#pragma unroll
+                    for (int d = 0; d < 3; ++d)
+#pragma unroll
+                        for (int h = 0; h < 2; ++h)
+                            ptx::bulk_g2s(sA + (2 * d + h) * DG_SLAB, a0 + h * t64_stride + (kk * 3 + d) * DG_SLAB, DG_SLAB,
+                                          FULL(stage));
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+                        ptx::bulk_g2s(sB + h * 3 * DG_SLAB, b0 + h * t64_stride + kk * 3 * DG_SLAB, 3 * DG_SLAB, FULL(stage));
+                    if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (warp-uniform loop, one elected lane issues) =====
+        constexpr uint32_t ID192 = ptx::idesc_s8(128, 192), ID128 = ptx::idesc_s8(128, 128), ID64 = ptx::idesc_s8(128, 64);
+        constexpr uint64_t DESC_HI = (uint64_t)((256u >> 4) | (1u << 14)) << 32;          // SBO 256 B, version 1
+        const uint32_t lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(smem) & 0x3FFFFu) >> 4);   // LBO 128 B
+        uint32_t stage = 0, phase = 0, tile_n = 0;
+        for (int64_t t = blockIdx.x; t < P.total; t += gridDim.x, ++tile_n) {
+            ptx::mbar_wait(ACC_EMPTY, (tile_n & 1) ^ 1);
+            ptx::tc_fence_after();
+            for (int64_t kk = 0; kk < ks; ++kk) {
+                ptx::mbar_wait(FULL(stage), phase);
+                ptx::tc_fence_after();
+                if (ptx::elect_one()) {
+                    const uint32_t a_lo = lo0 + stage * (DG_STAGE_BYTES >> 4);
+                    const uint32_t b_lo = a_lo + ((6 * DG_SLAB) >> 4);
+                    const uint32_t acc = kk > 0;
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const uint64_t db = DESC_HI | (b_lo + h * ((3 * DG_SLAB) >> 4));
+                        const uint32_t d = tmem + h * 192;
+                        ptx::mma_i8(d, DESC_HI | a_lo, db, ID192, acc);
+                        ptx::mma_i8(d + 64, DESC_HI | (a_lo + ((2 * DG_SLAB) >> 4)), db, ID128, 1);
+                        ptx::mma_i8(d + 128, DESC_HI | (a_lo + ((4 * DG_SLAB) >> 4)), db, ID64, 1);
+                    }
+                    ptx::tc_commit(EMPTY(stage));
+                    if (kk == ks - 1) ptx::tc_commit(ACC_FULL);
+                }
+                __syncwarp();
+                if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
+            }
+        }
+    } else {
+        // ===== epilogue: thread = row model (TMEM lane), loops over the 128 column models of the tile =====
+        const int quad = warp & 3;
+        uint32_t tile_n = 0;
+        for (int64_t t = blockIdx.x; t < P.total; t += gridDim.x, ++tile_n) {
+            int32_t I, J;
+            dg_tile_from_linear(t, P.T, I, J);
+            const int64_t i = (int64_t)I * DG_TILE + quad * 32 + lane;
+            const DStat si = P.stat[i];                          // slots beyond N hold neutral records
+            const double pwi = (double)si.pw * 0x1p-30;
+            const int64_t rowoff = i * (2 * P.N - i - 1) / 2 - i - 1;
+            ptx::mbar_wait(ACC_FULL, tile_n & 1);
+            ptx::tc_fence_after();
+            const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16);
+#pragma unroll 1
+            for (int c = 0; c < 8; ++c) {                        // 16-column chunks: half h = c / 4
+                const int h = c >> 2, cb = c & 3;
+                uint32_t v0[16], v1[16], v2[16];
+                ptx::tmem_ld_32x32b_x16(ta + h * 192 + 16 * cb, v0);
+                ptx::tmem_ld_32x32b_x16(ta + h * 192 + 64 + 16 * cb, v1);
+                ptx::tmem_ld_32x32b_x16(ta + h * 192 + 128 + 16 * cb, v2);
+                ptx::tmem_ld_wait();
+                const int64_t j0 = (int64_t)J * DG_TILE + h * DG_HALF + 16 * cb;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const int64_t j = j0 + e;
+                    if (i < P.N && j < P.N && j > i) {
+                        const DStat sj = P.stat[j];
+                        const long long dot = ((long long)(int32_t)v0[e] << 16) + ((long long)(int32_t)v1[e] << 8) +
+                                              (long long)(int32_t)v2[e];
+                        const double res = (si.T + sj.T) - 2.0 * (double)dot * (pwi * (double)sj.pw);
+                        const float d2 = (float)(res * P.invKk);
+                        P.out[rowoff + j] = sqrtf(d2 < 0.0f ? 0.0f : d2);    // clamp (NaN stays NaN)
+                    }
+                }
+            }
+            ptx::tc_fence_before();
+            __syncwarp();
+            if (lane == 0) ptx::mbar_arrive(ACC_EMPTY);
+        }
+    }
+    ptx::tc_fence_before();
+    __syncthreads();
+    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+}
+
+static inline size_t drmsd_smem_bytes() { return (size_t)DG_STAGES * DG_STAGE_BYTES + 8 * (2 * DG_STAGES + 2) + 16; }
+
+static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, float* out, char* ws, int sms, cudaStream_t s)
+{
+    const DWorkspace w = drmsd_workspace_layout(N, L);
+    DStat* stat = (DStat*)(ws + w.off_stat);
+    int8_t* plane = (int8_t*)(((uintptr_t)(ws + w.off_plane) + 255) & ~(uintptr_t)255);
+    drmsd_prep_kernel<<<(unsigned)(w.Np / DG_PREP_WARPS), DG_PREP_WARPS * 32, 0, s>>>(coords, N, L, w.K, w.ks, plane, stat);
+    CLUSCO_CUDA_TRY(cudaGetLastError());
+    DGParams P;
+    P.plane = plane;
+    P.stat = stat;
+    P.out = out;
+    P.N = N;
+    P.ks = w.ks;
+    P.T = (int32_t)(w.Np / DG_TILE);
+    P.total = (int64_t)P.T * (P.T + 1) / 2;
+    P.invKk = 1.0 / (DG_KAPPA * DG_KAPPA * (double)w.K);
+    const size_t smem = drmsd_smem_bytes();
+    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(drmsd_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const int64_t grid = P.total < sms ? P.total : sms;
+    drmsd_gram_kernel<<<(unsigned)grid, DG_THREADS, smem, s>>>(P);
+    CLUSCO_CUDA_TRY(cudaGetLastError());
+    return CLUSCO_OK;
+}
+
+}  // namespace clusco
