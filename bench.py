@@ -277,8 +277,11 @@ def main():
     if not args.no_ova and world == 1:
         ova = one_vs_all_side(clusco, wl, pk, flush)
     consumers = None
+    drmsd = None
     if not args.no_ova and world == 1:
         consumers = consumers_side(clusco, coords, ws, flush, P, ms_per_step)
+        del ws
+        drmsd = drmsd_side(clusco, coords, out, flush, N, L, P, pk)
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -294,7 +297,7 @@ def main():
                    "engine": {1: "ffma", 2: "i8tc"}[engine], "l2": "flushed between timed iterations (256 MB write)",
                    "effective_tflops": flops * world / (ms_per_step * 1e-3) / 1e12},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step(engine) * args.steps,
-        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova, "consumers": consumers,
+        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova, "consumers": consumers, "drmsd": drmsd,
     }))
     if dist:
         dist.destroy_process_group()
@@ -369,6 +372,38 @@ def consumers_side(clusco, coords, ws, flush, P, store_ms):
         if name.startswith("below"):
             res[name]["pairs_found"] = int(r[3].item())
     return res
+
+
+def drmsd_side(clusco, coords, out, flush, N, L, P, pk):
+    """NEXT-2: all-vs-all dRMSD (eq. 5) on the same ensemble -- one int8 tensor-core Gram over the
+    K = L(L-1)/2 distances per model.  Algorithmic work = 2 K flop per pair (one multiply-add per distance)."""
+    import torch
+    stream = torch.cuda.current_stream()
+    K = L * (L - 1) // 2
+    ws = torch.empty(int(clusco.load().clusco_drmsd_allpairs_workspace(N, L)), dtype=torch.uint8, device="cuda")
+    for _ in range(2):
+        clusco.clusco_drmsd_allpairs(coords, out, ws)
+    reps = 5
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    torch.cuda.synchronize()
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        clusco.clusco_drmsd_allpairs(coords, out, ws)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / reps
+    flops = 2.0 * K * P
+    peak = 2.0 * pk["bf16_tflops"]
+    Np = (N + 127) // 128 * 128
+    T = Np // 128
+    issued = 2.0 * (T * (T + 1) // 2) * ((K + 31) // 32) * 128 * (2 * (192 + 128 + 64)) * 32
+    return {"workload": f"dRMSD all-vs-all, N={N} x L={L} (K={K} distances per model)", "ms": ms,
+            "pairs_per_s": P / (ms * 1e-3),
+            "roofline": {"bound": "tensor", "achieved": flops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
+                         "frac": flops / (ms * 1e-3) / 1e12 / peak,
+                         "issued_frac": issued / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel (+ drmsd_prep_kernel)",
+                         "workspace_bytes": int(ws.numel())}}
 
 
 def launches_per_step(engine):
