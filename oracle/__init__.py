@@ -31,10 +31,16 @@ _LIB_D = os.path.join(_HERE, "libdrmsd_oracle.so")
 _lib_d = None
 
 
+_SRC_C = os.path.join(_HERE, "cmo_oracle.c")
+_LIB_C = os.path.join(_HERE, "libcmo_oracle.so")
+_lib_c = None
+
+
 def _compile(src: str, lib: str, force: bool) -> str:
     if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
         tmp = lib + f".tmp{os.getpid()}"
-        subprocess.run(["gcc", "-O2", "-fopenmp", "-shared", "-fPIC", "-o", tmp, src, "-lm"], check=True)
+        subprocess.run(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-o", tmp, src, "-lm"],
+                       check=True)
         os.replace(tmp, lib)
     return lib
 
@@ -42,6 +48,7 @@ def _compile(src: str, lib: str, force: bool) -> str:
 def build(force: bool = False) -> str:
     """Compile crmsd_oracle.c and drmsd_oracle.c (gcc -O2 -fopenmp, no fast-math); returns the cRMSD library."""
     _compile(_SRC_D, _LIB_D, force)
+    _compile(_SRC_C, _LIB_C, force)
     return _compile(_SRC, _LIB, force)
 
 
@@ -277,3 +284,56 @@ def drmsd_pairs(coords, pi, pj):
     d2 = np.empty(pi.size, np.float64)
     _load_d().oracle_drmsd_pairs(_p(x, _f32p), N, L, _p(pi, _i64p), _p(pj, _i64p), pi.size, _p(d, _f64p), _p(d2, _f64p))
     return d, d2
+
+
+# ---- CMO (oracle = eq. 6-7 literally, cmo_oracle.c) --------------------------------
+def _load_c():
+    global _lib_c
+    if _lib_c is None:
+        lib = ctypes.CDLL(_compile(_SRC_C, _LIB_C, False))
+        lib.oracle_cmo_pair.argtypes = [_f32p, _f32p, ctypes.c_int32, ctypes.c_double, _i64p]
+        lib.oracle_cmo_pair.restype = ctypes.c_double
+        lib.oracle_cmo_rows.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, ctypes.c_int64,
+                                        ctypes.c_int64, _f64p]
+        lib.oracle_cmo_rows.restype = None
+        lib.oracle_cmo_pairs.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, _i64p, _i64p,
+                                         ctypes.c_int64, _f64p]
+        lib.oracle_cmo_pairs.restype = None
+        _lib_c = lib
+    return _lib_c
+
+
+def _cut(cutoff):
+    return float(np.float32(cutoff))          # the C ABI takes the cut-off as fp32; both sides widen that value
+
+
+def cmo_pair(xa, xb, cutoff):
+    """eq. 6-7 for one pair: (S, [n(A), n(B), n(A and B)])."""
+    a, b = _f32(xa), _f32(xb)
+    cnt = np.zeros(3, np.int64)
+    s = _load_c().oracle_cmo_pair(_p(a, _f32p), _p(b, _f32p), a.shape[0], _cut(cutoff), _p(cnt, _i64p))
+    return float(s), cnt
+
+
+def cmo_rows(coords, cutoff, row_begin, row_end):
+    x = _f32(coords)
+    N, L, _ = x.shape
+    n = (row_begin * (2 * N - row_begin - 1) // 2, row_end * (2 * N - row_end - 1) // 2)
+    s = np.empty(n[1] - n[0], np.float64)
+    _load_c().oracle_cmo_rows(_p(x, _f32p), N, L, _cut(cutoff), int(row_begin), int(row_end), _p(s, _f64p))
+    return s
+
+
+def cmo_allpairs(coords, cutoff):
+    x = _f32(coords)
+    return cmo_rows(x, cutoff, 0, x.shape[0])
+
+
+def cmo_pairs(coords, cutoff, pi, pj):
+    x = _f32(coords)
+    N, L, _ = x.shape
+    pi = np.ascontiguousarray(pi, np.int64)
+    pj = np.ascontiguousarray(pj, np.int64)
+    s = np.empty(pi.size, np.float64)
+    _load_c().oracle_cmo_pairs(_p(x, _f32p), N, L, _cut(cutoff), _p(pi, _i64p), _p(pj, _i64p), pi.size, _p(s, _f64p))
+    return s
