@@ -148,6 +148,22 @@ int clusco_drmsd_allpairs(const float* coords, int64_t N, int32_t L, float* out,
                           void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * All-versus-all contact map overlap, the paper's eq. 6-7: with the binary contact map
+ *     C_ij = 1 if |x_i - x_j| < cutoff else 0      (i < j: contacts are pairs of distinct atoms; the paper gives
+ *                                                   no cut-off value, so it is an argument),
+ * the Sorensen similarity index  S = 100 * 2 n(A and B) / (n(A) + n(B)),  n(.) = number of contacts.
+ * out[N(N-1)/2]: packed row-major upper triangle, S in [0, 100].  Two maps with no contact at all are identical
+ * maps: S = 100 (0/0 is read that way; also every pair when L = 1).  The contact decision is taken in FP64 on the
+ * fp32 coordinates (sqrt(dx^2 + dy^2 + dz^2) < (double)cutoff, IEEE operations), the counts are exact integers
+ * (0/1 int8 operands, int32 tensor-core accumulation), S = (float)(200.0 * n_AB / (n_A + n_B)).
+ * Needs L <= 296 (shared-memory staging of a model), cutoff >= 0.  workspace: >= clusco_cmo_allpairs_workspace(N, L)
+ * bytes (about N L(L-1)/2 bytes), 256-byte aligned.  NaN/Inf coordinates -> NaN for that model's pairs.
+ */
+size_t clusco_cmo_allpairs_workspace(int64_t N, int32_t L);
+int clusco_cmo_allpairs(const float* coords, int64_t N, int32_t L, float cutoff, float* out,
+                        void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * One reference structure against N models: native[L][3], coords[N][L][3]
  * (neither pre-centred) -> out[N], out[k] = cRMSD(native, model k).
  */

@@ -26,7 +26,7 @@ EXPORTS = (
     "clusco_crmsd_one_vs_all", "clusco_crmsd_allpairs_host", "clusco_crmsd_one_vs_all_host",
     "clusco_partition_rows", "clusco_engine_supported", "clusco_allpairs_prepare", "clusco_allpairs_compute",
     "clusco_host_release", "clusco_crmsd_allpairs_below", "clusco_crmsd_rowstats",
-    "clusco_drmsd_allpairs_workspace", "clusco_drmsd_allpairs",
+    "clusco_drmsd_allpairs_workspace", "clusco_drmsd_allpairs", "clusco_cmo_allpairs_workspace", "clusco_cmo_allpairs",
 )
 
 
@@ -72,6 +72,9 @@ def load(build_if_missing: bool = False):
     lib.clusco_drmsd_allpairs_workspace.argtypes = [i64, i32]
     lib.clusco_drmsd_allpairs_workspace.restype = sz
     lib.clusco_drmsd_allpairs.argtypes = [vp, i64, i32, vp, vp, sz, vp]
+    lib.clusco_cmo_allpairs_workspace.argtypes = [i64, i32]
+    lib.clusco_cmo_allpairs_workspace.restype = sz
+    lib.clusco_cmo_allpairs.argtypes = [vp, i64, i32, ctypes.c_float, vp, vp, sz, vp]
     for name in EXPORTS:                       # every declared symbol must be exported
         getattr(lib, name)
     _lib = lib
@@ -232,6 +235,22 @@ def clusco_drmsd_allpairs(coords, out=None, workspace=None):
         st = load().clusco_drmsd_allpairs(_ptr(coords), N, L, _ptr(out), _ptr(workspace),
                                           workspace.numel() * workspace.element_size(), _stream_ptr(coords))
     _check(st, "clusco_drmsd_allpairs")
+    return out
+
+
+def clusco_cmo_allpairs(coords, cutoff: float, out=None, workspace=None):
+    """All-versus-all contact map overlap (eq. 6-7): packed upper triangle float32[N(N-1)/2] (include/clusco.h)."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    if out is None:
+        out = torch.empty(n_pairs(N), dtype=torch.float32, device=coords.device)
+    if workspace is None:
+        nbytes = int(load().clusco_cmo_allpairs_workspace(N, L))
+        workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=coords.device)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_cmo_allpairs(_ptr(coords), N, L, float(cutoff), _ptr(out), _ptr(workspace),
+                                        workspace.numel() * workspace.element_size(), _stream_ptr(coords))
+    _check(st, "clusco_cmo_allpairs")
     return out
 
 

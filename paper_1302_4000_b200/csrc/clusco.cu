@@ -29,6 +29,12 @@ static int check_device(int* sm_count)
 }
 
 static inline bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
+__global__ void fill_kernel(float* out, size_t n, float v)
+{
+    const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) out[k] = v;
+}
 }  // namespace clusco
 
 using namespace clusco;
@@ -281,7 +287,37 @@ int clusco_drmsd_allpairs(const float* coords, int64_t N, int32_t L, float* out,
     }
     const DWorkspace w = drmsd_workspace_layout(N, L);
     if (!workspace || workspace_bytes < w.total || ((uintptr_t)workspace & 255u)) return CLUSCO_ERR_WORKSPACE_TOO_SMALL;
-    return drmsd_launch(coords, N, L, out, (char*)workspace, sms, s);
+    return drmsd_launch<3>(coords, N, L, 0.0, out, (char*)workspace, sms, s);
+}
+
+// NEXT-3: all-versus-all contact-map overlap (eq. 6-7) as a 0/1 int8 Gram on the same kernels
+size_t clusco_cmo_allpairs_workspace(int64_t N, int32_t L)
+{
+    if (N < 0 || L < 1 || L > DG_MAX_L) return 0;
+    if (N < 2 || L < 2) return 256;
+    return drmsd_workspace_layout(N, L, 1).total;
+}
+
+int clusco_cmo_allpairs(const float* coords, int64_t N, int32_t L, float cutoff, float* out, void* workspace,
+                        size_t workspace_bytes, void* stream)
+{
+    if (N < 0 || L < 1 || L > DG_MAX_L || !(cutoff >= 0.0f)) return CLUSCO_ERR_INVALID_ARG;
+    if (N < 2) return CLUSCO_OK;
+    if (!coords || !out) return CLUSCO_ERR_INVALID_ARG;
+    if (N > (int64_t)1 << 24) return CLUSCO_ERR_INVALID_ARG;
+    int sms = 0;
+    int st = check_device(&sms);
+    if (st != CLUSCO_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (L < 2) {                                                // no atom pair: two empty maps, S = 100 (header)
+        const size_t n = (size_t)(N * (N - 1) / 2);
+        fill_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(out, n, 100.0f);
+        CLUSCO_CUDA_TRY(cudaGetLastError());
+        return CLUSCO_OK;
+    }
+    const DWorkspace w = drmsd_workspace_layout(N, L, 1);
+    if (!workspace || workspace_bytes < w.total || ((uintptr_t)workspace & 255u)) return CLUSCO_ERR_WORKSPACE_TOO_SMALL;
+    return drmsd_launch<1>(coords, N, L, (double)cutoff, out, (char*)workspace, sms, s);
 }
 
 // one launch, no scratch: every CTA centres the native into its own shared memory

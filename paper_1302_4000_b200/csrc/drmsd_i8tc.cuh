@@ -30,8 +30,12 @@ constexpr double DG_KAPPA = 127.0 / 128.0;
 constexpr int DG_MAX_L = 296;                  // 3 K 2^14 < 2^31 with K = L(L-1)/2
 constexpr int DG_TILE = 128, DG_HALF = 64;
 constexpr int DG_SLAB = 2048;                  // bytes of one (tile64, k-step, digit) image: 64 rows x 32 entries
-constexpr int DG_STAGE_BYTES = 3 * 2 * DG_SLAB + 2 * 3 * DG_SLAB;   // A (3 digits x 128 rows) + B (2 halves x 3 digits x 64)
-constexpr int DG_STAGES = 8;
+// DIGITS = 3: dRMSD (24-bit fixed-point distances); DIGITS = 1: CMO (0/1 contact maps, eq. 6-7) on the same kernels
+template <int DIGITS> struct DGCfg {
+    static constexpr int STAGE_BYTES = DIGITS * 2 * DG_SLAB + 2 * DIGITS * DG_SLAB;   // A (digits x 128 rows) + B (2 halves x digits x 64)
+    static constexpr int STAGES = DIGITS == 3 ? 8 : 24;
+    static constexpr int HALF_COLS = 64 * DIGITS;                                      // TMEM columns per 64-model half
+};
 constexpr int DG_THREADS = 6 * 32;
 constexpr int DG_PREP_WARPS = 8;
 
@@ -45,7 +49,7 @@ struct DWorkspace {
     int64_t N, Np, K, ks, tiles64;
     size_t off_stat, off_plane, total;
 };
-static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L)
+static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L, int digits = 3)
 {
     DWorkspace w;
     w.N = N;
@@ -57,7 +61,7 @@ static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L)
     w.off_stat = o;
     o += (size_t)round_up((int64_t)sizeof(DStat) * w.Np, 256);
     w.off_plane = o;
-    o += (size_t)round_up(w.tiles64 * w.ks * 3 * DG_SLAB, 256);
+    o += (size_t)round_up(w.tiles64 * w.ks * digits * DG_SLAB, 256);
     w.total = o + 256;
     return w;
 }
@@ -65,9 +69,12 @@ static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L)
 // ---- distances, scale, digits, operand plane: one CTA per 8 consecutive models (one core-matrix row group), one
 // warp per model; lane = entry within the k-step.  Two passes over the K distances (max, then quantise), each
 // recomputed in FP64 from the fp32 coordinates held in shared memory.
+// DIGITS = 1 (CMO): the entry is the contact bit C_ij = (|x_i - x_j| < cutoff), eq. 6 -- decided in FP64 with IEEE
+// operations only (no FMA contraction), so the decision is reproducible bit for bit; T = n(A), the contact count.
+template <int DIGITS>
 __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const float* __restrict__ coords, int64_t N, int32_t L,
-                                                                        int64_t K, int64_t ks, int8_t* __restrict__ plane,
-                                                                        DStat* __restrict__ stat)
+                                                                        int64_t K, int64_t ks, double cutoff,
+                                                                        int8_t* __restrict__ plane, DStat* __restrict__ stat)
 {
     __shared__ float xs[DG_PREP_WARPS][3 * DG_MAX_L];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -85,11 +92,11 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         const double dx = (double)x[3 * i] - (double)x[3 * j];
         const double dy = (double)x[3 * i + 1] - (double)x[3 * j + 1];
         const double dz = (double)x[3 * i + 2] - (double)x[3 * j + 2];
-        return dx * dx + dy * dy + dz * dz;
+        return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
     };
     // pass 1: largest distance -> power-of-two scale with dmax 2^-ex in [0.5, 1)
     double m2 = 0.0;
-    if (valid) {
+    if (valid && DIGITS == 3) {
         int i = 0, pos = lane;                                   // entry k = lane, lane + 32, ...: pair (i, i + 1 + pos)
         for (int64_t k = lane; k < K; k += 32) {
             while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
@@ -109,7 +116,7 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
     const int64_t t64 = n >> 6;
     const int g = (int)(n & 63) >> 3, r8 = (int)(n & 7);
     const int kc = lane >> 4, kb = lane & 15;
-    int8_t* base = plane + (t64 * ks * 3) * DG_SLAB + g * 256 + kc * 128 + r8 * 16 + kb;
+    int8_t* base = plane + (t64 * ks * DIGITS) * DG_SLAB + g * 256 + kc * 128 + r8 * 16 + kb;
     long long sumsq = 0ll;
     int i = 0, pos = lane;
     for (int64_t kk = 0; kk < ks; ++kk) {
@@ -117,8 +124,14 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         int I = 0;
         if (valid && k < K) {
             while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
-            I = __double2int_rn(sqrt(dist2(i, i + 1 + pos)) * scale);
+            const double d = sqrt(dist2(i, i + 1 + pos));
+            I = DIGITS == 3 ? __double2int_rn(d * scale) : (d < cutoff ? 1 : 0);
             pos += 32;
+        }
+        if (DIGITS == 1) {
+            sumsq += I;
+            base[kk * DG_SLAB] = (int8_t)I;
+            continue;
         }
         const int g2 = (int)(int8_t)(I & 0xff);
         const int I1 = (I - g2) >> 8;
@@ -137,8 +150,8 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
     finite = __all_sync(0xffffffffu, finite);
     if (lane == 0) {
         DStat s;
-        s.T = ldexp((double)sumsq, 2 * ex - 46);
-        if (!finite || !in_range) s.T = __longlong_as_double(0x7ff8000000000000ll);
+        s.T = DIGITS == 3 ? ldexp((double)sumsq, 2 * ex - 46) : (double)sumsq;
+        if (!finite || (DIGITS == 3 && !in_range)) s.T = __longlong_as_double(0x7ff8000000000000ll);
         s.pw = pow2i(ex);
         s.pad = 0.0f;
         stat[n] = s;
@@ -168,8 +181,11 @@ __device__ __forceinline__ void dg_tile_from_linear(int64_t t, int32_t T, int32_
     J = I + (int32_t)(t - ((int64_t)I * T - (int64_t)I * (I - 1) / 2));
 }
 
+template <int DIGITS>
 __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParams P)
 {
+    constexpr int DG_STAGES = DGCfg<DIGITS>::STAGES, DG_STAGE_BYTES = DGCfg<DIGITS>::STAGE_BYTES;
+    constexpr int HC = DGCfg<DIGITS>::HALF_COLS;
     extern __shared__ __align__(128) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)DG_STAGES * DG_STAGE_BYTES);
     const uint32_t bar0 = ptx::smem_u32(bars);
@@ -202,23 +218,24 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
             for (int64_t t = blockIdx.x; t < P.total; t += gridDim.x) {
                 int32_t I, J;
                 dg_tile_from_linear(t, P.T, I, J);
-                const int8_t* a0 = P.plane + ((int64_t)(2 * I) * ks * 3) * DG_SLAB;       // tile64 2I; 2I + 1 follows at + ks * 3 slabs
-                const int8_t* b0 = P.plane + ((int64_t)(2 * J) * ks * 3) * DG_SLAB;
-                const int64_t t64_stride = ks * 3 * DG_SLAB;
+                const int8_t* a0 = P.plane + ((int64_t)(2 * I) * ks * DIGITS) * DG_SLAB;  // tile64 2I; 2I + 1 follows at + ks * DIGITS slabs
+                const int8_t* b0 = P.plane + ((int64_t)(2 * J) * ks * DIGITS) * DG_SLAB;
+                const int64_t t64_stride = ks * DIGITS * DG_SLAB;
                 for (int64_t kk = 0; kk < ks; ++kk) {
                     ptx::mbar_wait(EMPTY(stage), phase ^ 1);
                     ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
                     const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
-                    const uint32_t sB = sA + 6 * DG_SLAB;
+                    const uint32_t sB = sA + 2 * DIGITS * DG_SLAB;
 #pragma unroll
-                    for (int d = 0; d < 3; ++d)
+                    for (int d = 0; d < DIGITS; ++d)
 #pragma unroll
                         for (int h = 0; h < 2; ++h)
-                            ptx::bulk_g2s(sA + (2 * d + h) * DG_SLAB, a0 + h * t64_stride + (kk * 3 + d) * DG_SLAB, DG_SLAB,
+                            ptx::bulk_g2s(sA + (2 * d + h) * DG_SLAB, a0 + h * t64_stride + (kk * DIGITS + d) * DG_SLAB, DG_SLAB,
                                           FULL(stage));
 #pragma unroll
                     for (int h = 0; h < 2; ++h)
-                        ptx::bulk_g2s(sB + h * 3 * DG_SLAB, b0 + h * t64_stride + kk * 3 * DG_SLAB, 3 * DG_SLAB, FULL(stage));
+                        ptx::bulk_g2s(sB + h * DIGITS * DG_SLAB, b0 + h * t64_stride + kk * DIGITS * DG_SLAB, DIGITS * DG_SLAB,
+                                      FULL(stage));
                     if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
                 }
             }
@@ -237,15 +254,19 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                 ptx::tc_fence_after();
                 if (ptx::elect_one()) {
                     const uint32_t a_lo = lo0 + stage * (DG_STAGE_BYTES >> 4);
-                    const uint32_t b_lo = a_lo + ((6 * DG_SLAB) >> 4);
+                    const uint32_t b_lo = a_lo + ((2 * DIGITS * DG_SLAB) >> 4);
                     const uint32_t acc = kk > 0;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        const uint64_t db = DESC_HI | (b_lo + h * ((3 * DG_SLAB) >> 4));
-                        const uint32_t d = tmem + h * 192;
-                        ptx::mma_i8(d, DESC_HI | a_lo, db, ID192, acc);
-                        ptx::mma_i8(d + 64, DESC_HI | (a_lo + ((2 * DG_SLAB) >> 4)), db, ID128, 1);
-                        ptx::mma_i8(d + 128, DESC_HI | (a_lo + ((4 * DG_SLAB) >> 4)), db, ID64, 1);
+                        const uint64_t db = DESC_HI | (b_lo + h * ((DIGITS * DG_SLAB) >> 4));
+                        const uint32_t d = tmem + h * HC;
+                        if (DIGITS == 3) {
+                            ptx::mma_i8(d, DESC_HI | a_lo, db, ID192, acc);
+                            ptx::mma_i8(d + 64, DESC_HI | (a_lo + ((2 * DG_SLAB) >> 4)), db, ID128, 1);
+                            ptx::mma_i8(d + 128, DESC_HI | (a_lo + ((4 * DG_SLAB) >> 4)), db, ID64, 1);
+                        } else {
+                            ptx::mma_i8(d, DESC_HI | a_lo, db, ID64, acc);
+                        }
                     }
                     ptx::tc_commit(EMPTY(stage));
                     if (kk == ks - 1) ptx::tc_commit(ACC_FULL);
@@ -272,9 +293,11 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
             for (int c = 0; c < 8; ++c) {                        // 16-column chunks: half h = c / 4
                 const int h = c >> 2, cb = c & 3;
                 uint32_t v0[16], v1[16], v2[16];
-                ptx::tmem_ld_32x32b_x16(ta + h * 192 + 16 * cb, v0);
-                ptx::tmem_ld_32x32b_x16(ta + h * 192 + 64 + 16 * cb, v1);
-                ptx::tmem_ld_32x32b_x16(ta + h * 192 + 128 + 16 * cb, v2);
+                ptx::tmem_ld_32x32b_x16(ta + h * HC + 16 * cb, v0);
+                if (DIGITS == 3) {
+                    ptx::tmem_ld_32x32b_x16(ta + h * HC + 64 + 16 * cb, v1);
+                    ptx::tmem_ld_32x32b_x16(ta + h * HC + 128 + 16 * cb, v2);
+                }
                 ptx::tmem_ld_wait();
                 const int64_t j0 = (int64_t)J * DG_TILE + h * DG_HALF + 16 * cb;
 #pragma unroll
@@ -282,11 +305,19 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                     const int64_t j = j0 + e;
                     if (i < P.N && j < P.N && j > i) {
                         const DStat sj = P.stat[j];
-                        const long long dot = ((long long)(int32_t)v0[e] << 16) + ((long long)(int32_t)v1[e] << 8) +
-                                              (long long)(int32_t)v2[e];
-                        const double res = (si.T + sj.T) - 2.0 * (double)dot * (pwi * (double)sj.pw);
-                        const float d2 = (float)(res * P.invKk);
-                        P.out[rowoff + j] = sqrtf(d2 < 0.0f ? 0.0f : d2);    // clamp (NaN stays NaN)
+                        if (DIGITS == 3) {
+                            const long long dot = ((long long)(int32_t)v0[e] << 16) + ((long long)(int32_t)v1[e] << 8) +
+                                                  (long long)(int32_t)v2[e];
+                            const double res = (si.T + sj.T) - 2.0 * (double)dot * (pwi * (double)sj.pw);
+                            const float d2 = (float)(res * P.invKk);
+                            P.out[rowoff + j] = sqrtf(d2 < 0.0f ? 0.0f : d2);    // clamp (NaN stays NaN)
+                        } else {
+                            // eq. 7: S = 100 * 2 n(A and B) / (n(A) + n(B)); two empty maps are identical: 100
+                            const double den = si.T + sj.T;
+                            const double S = den > 0.0 ? __ddiv_rn(__dmul_rn(200.0, (double)(int32_t)v0[e]), den)
+                                                       : (den == 0.0 ? 100.0 : den);          // NaN model -> NaN
+                            P.out[rowoff + j] = (float)S;
+                        }
                     }
                 }
             }
@@ -300,14 +331,15 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
 }
 
-static inline size_t drmsd_smem_bytes() { return (size_t)DG_STAGES * DG_STAGE_BYTES + 8 * (2 * DG_STAGES + 2) + 16; }
-
-static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, float* out, char* ws, int sms, cudaStream_t s)
+template <int DIGITS>
+static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double cutoff, float* out, char* ws, int sms,
+                               cudaStream_t s)
 {
-    const DWorkspace w = drmsd_workspace_layout(N, L);
+    const DWorkspace w = drmsd_workspace_layout(N, L, DIGITS);
     DStat* stat = (DStat*)(ws + w.off_stat);
-    int8_t* plane = (int8_t*)(((uintptr_t)(ws + w.off_plane) + 255) & ~(uintptr_t)255);
-    drmsd_prep_kernel<<<(unsigned)(w.Np / DG_PREP_WARPS), DG_PREP_WARPS * 32, 0, s>>>(coords, N, L, w.K, w.ks, plane, stat);
+    int8_t* plane = (int8_t*)(ws + w.off_plane);
+    drmsd_prep_kernel<DIGITS><<<(unsigned)(w.Np / DG_PREP_WARPS), DG_PREP_WARPS * 32, 0, s>>>(coords, N, L, w.K, w.ks, cutoff,
+                                                                                              plane, stat);
     CLUSCO_CUDA_TRY(cudaGetLastError());
     DGParams P;
     P.plane = plane;
@@ -318,10 +350,10 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, float*
     P.T = (int32_t)(w.Np / DG_TILE);
     P.total = (int64_t)P.T * (P.T + 1) / 2;
     P.invKk = 1.0 / (DG_KAPPA * DG_KAPPA * (double)w.K);
-    const size_t smem = drmsd_smem_bytes();
-    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(drmsd_gram_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t smem = (size_t)DGCfg<DIGITS>::STAGES * DGCfg<DIGITS>::STAGE_BYTES + 8 * (2 * DGCfg<DIGITS>::STAGES + 2) + 16;
+    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(drmsd_gram_kernel<DIGITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t grid = P.total < sms ? P.total : sms;
-    drmsd_gram_kernel<<<(unsigned)grid, DG_THREADS, smem, s>>>(P);
+    drmsd_gram_kernel<DIGITS><<<(unsigned)grid, DG_THREADS, smem, s>>>(P);
     CLUSCO_CUDA_TRY(cudaGetLastError());
     return CLUSCO_OK;
 }

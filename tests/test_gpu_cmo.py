@@ -1,0 +1,80 @@
+"""GPU parity of the CMO path (eq. 6-7) against the oracle (oracle/cmo_oracle.c).
+
+Integer work: the contact decisions are taken in FP64 with the same IEEE operations on both sides and the counts are
+exact, and S = (float)(200.0 * n_AB / (n_A + n_B)) is one correctly rounded division -- so the bar is BIT-EXACT
+equality with the oracle's value rounded to fp32.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1302_4000_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def clusco():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: -m gpu tests need the B200 box")
+    import paper_1302_4000_b200 as pkg
+    pkg.load()
+    return pkg
+
+
+def _dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+@pytest.mark.parametrize("cfg,N,cutoff", [("C1", None, 8.0), ("C2", 300, 6.5), ("C3", 200, 10.0), ("C1", 150, 3.9)])
+def test_cmo_every_pair_bit_exact(clusco, cfg, N, cutoff):
+    ens = wl.make_config(cfg, N=N)
+    want = oracle.cmo_allpairs(ens.coords, cutoff).astype(np.float32)
+    got = clusco.clusco_cmo_allpairs(_dev(ens.coords), cutoff).cpu().numpy()
+    assert np.array_equal(got, want), (cfg, np.abs(got - want).max())
+    assert want.min() < 99.0 and want.max() <= 100.0
+
+
+@pytest.mark.parametrize("N,L", [(2, 2), (3, 5), (129, 33), (257, 64), (130, 296)])
+def test_cmo_ragged_shapes(clusco, N, L):
+    rng = np.random.default_rng(N * 1000 + L)
+    x = (rng.normal(size=(N, L, 3)) * 6 + rng.uniform(-40, 40, size=(N, 1, 3))).astype(np.float32)
+    x[1] = x[0]
+    want = oracle.cmo_allpairs(x, 7.0).astype(np.float32)
+    got = clusco.clusco_cmo_allpairs(_dev(x), 7.0).cpu().numpy()
+    assert np.array_equal(got, want)
+    assert got[0] == 100.0
+
+
+def test_cmo_edge_cases(clusco):
+    import torch
+    x = _dev(wl.make_config("C1").coords)
+    assert clusco.clusco_cmo_allpairs(x[:1].contiguous(), 8.0).numel() == 0
+    assert torch.all(clusco.clusco_cmo_allpairs(x[:5, :1, :].contiguous(), 8.0) == 100.0)      # no atom pair
+    assert torch.all(clusco.clusco_cmo_allpairs(x[:9].contiguous(), 0.0) == 100.0)             # no contact at all
+    assert torch.all(clusco.clusco_cmo_allpairs(x[:9].contiguous(), 1e9) == 100.0)             # every pair in contact
+    with pytest.raises(clusco.CluscoError):
+        clusco.clusco_cmo_allpairs(x[:4].contiguous(), -1.0)
+    y = x[:40].clone()
+    y[7, 2, 0] = float("nan")
+    got = clusco.clusco_cmo_allpairs(y, 8.0).cpu().numpy()
+    bad = np.zeros(got.size, bool)
+    for j in range(40):
+        if j != 7:
+            bad[wl.packed_index(min(7, j), max(7, j), 40)] = True
+    assert np.all(np.isnan(got[bad])) and np.all(np.isfinite(got[~bad]))
+
+
+def test_cmo_full_size_sampled(clusco):
+    """C3 at full size (10000 x 250), sampled pairs one by one."""
+    ens = wl.make_config("C3")
+    got = clusco.clusco_cmo_allpairs(_dev(ens.coords), 8.0).cpu().numpy()
+    rng = np.random.default_rng(11)
+    pi = rng.integers(0, ens.N - 1, 400)
+    pj = np.array([rng.integers(i + 1, ens.N) for i in pi])
+    pi = np.concatenate([pi, [0, 0, ens.N - 2, 127, 128]])
+    pj = np.concatenate([pj, [1, ens.N - 1, ens.N - 1, 128, 9999]])
+    want = oracle.cmo_pairs(ens.coords, 8.0, pi, pj).astype(np.float32)
+    assert np.array_equal(got[wl.packed_index(pi, pj, ens.N)], want)
