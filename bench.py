@@ -278,10 +278,12 @@ def main():
         ova = one_vs_all_side(clusco, wl, pk, flush)
     consumers = None
     drmsd = None
+    cmo = None
     if not args.no_ova and world == 1:
         consumers = consumers_side(clusco, coords, ws, flush, P, ms_per_step)
         del ws
         drmsd = drmsd_side(clusco, coords, out, flush, N, L, P, pk)
+        cmo = cmo_side(clusco, coords, out, flush, N, L, P, pk)
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -297,7 +299,7 @@ def main():
                    "engine": {1: "ffma", 2: "i8tc"}[engine], "l2": "flushed between timed iterations (256 MB write)",
                    "effective_tflops": flops * world / (ms_per_step * 1e-3) / 1e12},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step(engine) * args.steps,
-        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova, "consumers": consumers, "drmsd": drmsd,
+        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova, "consumers": consumers, "drmsd": drmsd, "cmo": cmo,
     }))
     if dist:
         dist.destroy_process_group()
@@ -403,6 +405,35 @@ def drmsd_side(clusco, coords, out, flush, N, L, P, pk):
             "roofline": {"bound": "tensor", "achieved": flops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
                          "frac": flops / (ms * 1e-3) / 1e12 / peak,
                          "issued_frac": issued / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel (+ drmsd_prep_kernel)",
+                         "workspace_bytes": int(ws.numel())}}
+
+
+def cmo_side(clusco, coords, out, flush, N, L, P, pk):
+    """NEXT-3: all-vs-all contact map overlap (eq. 6-7, cut-off 8 A) on the same ensemble -- a 0/1
+    int8 tensor-core Gram over the K = L(L-1)/2 contact bits per model.  The operands are one byte per contact bit
+    (K N bytes), streamed tile by tile: the bound is operand delivery (HBM/L2), so the roofline is bytes."""
+    import torch
+    stream = torch.cuda.current_stream()
+    K = L * (L - 1) // 2
+    ws = torch.empty(int(clusco.load().clusco_cmo_allpairs_workspace(N, L)), dtype=torch.uint8, device="cuda")
+    for _ in range(2):
+        clusco.clusco_cmo_allpairs(coords, 8.0, out, ws)
+    reps = 5
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    torch.cuda.synchronize()
+    for a, b in ev:
+        flush.zero_()
+        a.record(stream)
+        clusco.clusco_cmo_allpairs(coords, 8.0, out, ws)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / reps
+    ops = 2.0 * K * P                                   # one AND + one add per contact bit and pair
+    peak = 2.0 * pk["bf16_tflops"]
+    return {"workload": f"CMO all-vs-all, cut-off 8 A, N={N} x L={L} (K={K} contact bits per model)", "ms": ms,
+            "pairs_per_s": P / (ms * 1e-3),
+            "roofline": {"bound": "tensor", "achieved": ops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TOP/s",
+                         "frac": ops / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel<1> (+ drmsd_prep_kernel<1>)",
                          "workspace_bytes": int(ws.numel())}}
 
 
