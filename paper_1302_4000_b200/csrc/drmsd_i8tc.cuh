@@ -38,6 +38,10 @@ template <int DIGITS> struct DGCfg {
 };
 constexpr int DG_THREADS = 6 * 32;
 constexpr int DG_PREP_WARPS = 8;
+#ifndef DG_CLUSTER_I
+#define DG_CLUSTER_I 2                         // cluster shape of the Gram kernel: CLI tile rows x CLJ tile columns
+#define DG_CLUSTER_J 2                         // (measured at C3's shape: 2x2 7.46 ms, 1x2 7.78 ms, 2x1 9.25 ms, none 8.24 ms)
+#endif
 
 struct __align__(16) DStat {
     double T;          // KAPPA^2 sum_k d_k^2 of the quantised distances, true scale (Angstrom^2); NaN poisons the model
@@ -47,7 +51,7 @@ struct __align__(16) DStat {
 
 struct DWorkspace {
     int64_t N, Np, K, ks, tiles64;
-    size_t off_stat, off_plane, total;
+    size_t off_stat, off_sched, off_plane, total;
 };
 static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L, int digits = 3)
 {
@@ -60,6 +64,11 @@ static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L, int digits
     size_t o = 0;
     w.off_stat = o;
     o += (size_t)round_up((int64_t)sizeof(DStat) * w.Np, 256);
+    w.off_sched = o;                                       // int2 (SI, SJ) per super-tile of the cluster kernel's walk
+    {
+        const int64_t T = w.Np / DG_TILE;                  // at most T (T + 1) / 2 + T entries for any cluster shape
+        o += (size_t)round_up((int64_t)sizeof(int2) * (T * (T + 1) / 2 + T), 256);
+    }
     w.off_plane = o;
     o += (size_t)round_up(w.tiles64 * w.ks * digits * DG_SLAB, 256);
     w.total = o + 256;
@@ -162,10 +171,12 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
 struct DGParams {
     const int8_t* plane;
     const DStat* stat;
+    const int2* sched;     // cluster kernel: the super-tile walk (dg_schedule_kernel)
     float* out;
     int64_t N, ks;
     int32_t T;             // tiles per side (Np / 128); upper-triangle tiles I <= J are linearised row-major
     int64_t total;         // T (T + 1) / 2
+    int64_t n_sched;       // entries of `sched`
     double invKk;          // 1 / (KAPPA^2 K)
 };
 
@@ -181,9 +192,46 @@ __device__ __forceinline__ void dg_tile_from_linear(int64_t t, int32_t T, int32_
     J = I + (int32_t)(t - ((int64_t)I * T - (int64_t)I * (I - 1) / 2));
 }
 
-template <int DIGITS>
+// The cluster kernel's walk over the super-tiles that touch the upper triangle, in blocks of bi x bj super-tiles that
+// are about square in tile units and about one wave of clusters large: the clusters running at the same time then
+// share their A tile rows AND their B tile columns in L2 (a row-major walk shares one A row and streams every B
+// column from HBM: 18.5 GB of DRAM reads at C3's shape instead of 9.7 GB).  One thread, ~T^2/2 entries.
+// super-tile (SI, SJ) = tiles (cli SI + ri, clj SJ + rj); it is walked if any of its tiles lies on or above the diagonal
+__host__ __device__ __forceinline__ bool dg_super_valid(int32_t SI, int32_t SJ, int32_t cli, int32_t clj, int32_t T)
+{
+    return cli * SI < T && clj * SJ < T && cli * SI <= clj * SJ + (clj - 1);
+}
+__global__ void dg_schedule_kernel(int32_t T, int32_t cli, int32_t clj, int32_t bi, int32_t bj, int2* __restrict__ sched)
+{
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int32_t TI = (T + cli - 1) / cli, TJ = (T + clj - 1) / clj;
+    int64_t n = 0;
+    for (int32_t BI = 0; BI * bi < TI; ++BI)
+        for (int32_t BJ = 0; BJ * bj < TJ; ++BJ)
+            for (int32_t si = 0; si < bi; ++si)
+                for (int32_t sj = 0; sj < bj; ++sj) {
+                    const int32_t SI = BI * bi + si, SJ = BJ * bj + sj;
+                    if (SI < TI && SJ < TJ && dg_super_valid(SI, SJ, cli, clj, T)) sched[n++] = make_int2(SI, SJ);
+                }
+}
+static inline int64_t dg_schedule_count(int32_t T, int32_t cli, int32_t clj)
+{
+    const int32_t TI = (T + cli - 1) / cli, TJ = (T + clj - 1) / clj;
+    int64_t n = 0;
+    for (int32_t SI = 0; SI < TI; ++SI)
+        for (int32_t SJ = 0; SJ < TJ; ++SJ) n += dg_super_valid(SI, SJ, cli, clj, T) ? 1 : 0;
+    return n;
+}
+
+// CLI x CLJ = 1 x 1: every CTA fetches its own operands.  Otherwise thread-block clusters: the CTAs of a cluster work
+// on the CLI x CLJ block of tiles (CLI SI + ri, CLJ SJ + rj), rank = CLJ ri + rj; the A slabs of a tile row are needed
+// by the CTAs of that row and the B slabs of a tile column by the CTAs of that column, so with 2 x 2 each CTA fetches
+// HALF of its A and HALF of its B and multicasts them to its row / column partner: the L2 -> SM operand bytes halve.
+// A stage is free again when every CTA of the cluster has consumed it (EMPTY counts CL multicast commits).
+template <int DIGITS, int CLI, int CLJ>
 __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParams P)
 {
+    constexpr int CL = CLI * CLJ;                                // CTAs per cluster: CLI tile rows x CLJ tile columns
     constexpr int DG_STAGES = DGCfg<DIGITS>::STAGES, DG_STAGE_BYTES = DGCfg<DIGITS>::STAGE_BYTES;
     constexpr int HC = DGCfg<DIGITS>::HALF_COLS;
     extern __shared__ __align__(128) uint8_t smem[];
@@ -195,10 +243,12 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * DG_STAGES + 2);
 
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
+    const uint32_t rank = CL > 1 ? ptx::cluster_ctarank() : 0u;
+    const int ri = (int)(rank / CLJ), rj = (int)(rank % CLJ);
     if (threadIdx.x == 0) {
         for (int s = 0; s < DG_STAGES; ++s) {
             ptx::mbar_init(FULL(s), 1);
-            ptx::mbar_init(EMPTY(s), 1);
+            ptx::mbar_init(EMPTY(s), CL);
         }
         ptx::mbar_init(ACC_FULL, 1);
         ptx::mbar_init(ACC_EMPTY, 4);
@@ -207,35 +257,56 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
     if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
     ptx::tc_fence_before();
     __syncthreads();
+    if (CL > 1) ptx::cluster_sync();                             // every CTA's barriers exist before any remote signal
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
     const int64_t ks = P.ks;
+    // CL == 1: tiles I <= J row-major (dg_tile_from_linear); CL > 1: the super-tile list written by dg_schedule_kernel
+    const int64_t total2 = CL > 1 ? P.n_sched : P.total;
+    const int64_t first = blockIdx.x / CL, step = gridDim.x / CL;
 
     if (warp == 0) {
         // ===== producer =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
-            for (int64_t t = blockIdx.x; t < P.total; t += gridDim.x) {
-                int32_t I, J;
-                dg_tile_from_linear(t, P.T, I, J);
-                const int8_t* a0 = P.plane + ((int64_t)(2 * I) * ks * DIGITS) * DG_SLAB;  // tile64 2I; 2I + 1 follows at + ks * DIGITS slabs
-                const int8_t* b0 = P.plane + ((int64_t)(2 * J) * ks * DIGITS) * DG_SLAB;
-                const int64_t t64_stride = ks * DIGITS * DG_SLAB;
+            const int64_t t64_stride = ks * DIGITS * DG_SLAB;
+            for (int64_t t = first; t < total2; t += step) {
+                int32_t SI, SJ;
+                if (CL > 1) { const int2 e = P.sched[t]; SI = e.x; SJ = e.y; } else dg_tile_from_linear(t, P.T, SI, SJ);
+                const int32_t I = min(CLI * SI + ri, P.T - 1), J = min(CLJ * SJ + rj, P.T - 1);   // clamped: results are masked
+                const int8_t* a0 = P.plane + (int64_t)(2 * I) * t64_stride;               // tile64 2I; 2I + 1 follows
+                const int8_t* b0 = P.plane + (int64_t)(2 * J) * t64_stride;
                 for (int64_t kk = 0; kk < ks; ++kk) {
                     ptx::mbar_wait(EMPTY(stage), phase ^ 1);
                     ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
                     const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
                     const uint32_t sB = sA + 2 * DIGITS * DG_SLAB;
+                    // A tile: needed by the CLJ CTAs of my tile row -- with CLJ == 2 I fetch half rj and multicast it
+                    if (CLJ == 2) {
+                        const uint16_t row_mask = (uint16_t)(3u << (ri * CLJ));
 #pragma unroll
-                    for (int d = 0; d < DIGITS; ++d)
+                        for (int d = 0; d < DIGITS; ++d)
+                            ptx::bulk_g2s_multicast(sA + (2 * d + rj) * DG_SLAB, a0 + rj * t64_stride + (kk * DIGITS + d) * DG_SLAB,
+                                                    DG_SLAB, FULL(stage), row_mask);
+                    } else {
+#pragma unroll
+                        for (int d = 0; d < DIGITS; ++d)
+#pragma unroll
+                            for (int h = 0; h < 2; ++h)
+                                ptx::bulk_g2s(sA + (2 * d + h) * DG_SLAB, a0 + h * t64_stride + (kk * DIGITS + d) * DG_SLAB,
+                                              DG_SLAB, FULL(stage));
+                    }
+                    // B tile: needed by the CLI CTAs of my tile column -- with CLI == 2 I fetch half ri and multicast it
+                    if (CLI == 2) {
+                        const uint16_t col_mask = (uint16_t)((1u | (1u << CLJ)) << rj);
+                        ptx::bulk_g2s_multicast(sB + ri * DIGITS * DG_SLAB, b0 + ri * t64_stride + kk * DIGITS * DG_SLAB,
+                                                DIGITS * DG_SLAB, FULL(stage), col_mask);
+                    } else {
 #pragma unroll
                         for (int h = 0; h < 2; ++h)
-                            ptx::bulk_g2s(sA + (2 * d + h) * DG_SLAB, a0 + h * t64_stride + (kk * DIGITS + d) * DG_SLAB, DG_SLAB,
-                                          FULL(stage));
-#pragma unroll
-                    for (int h = 0; h < 2; ++h)
-                        ptx::bulk_g2s(sB + h * DIGITS * DG_SLAB, b0 + h * t64_stride + kk * DIGITS * DG_SLAB, DIGITS * DG_SLAB,
-                                      FULL(stage));
+                            ptx::bulk_g2s(sB + h * DIGITS * DG_SLAB, b0 + h * t64_stride + kk * DIGITS * DG_SLAB,
+                                          DIGITS * DG_SLAB, FULL(stage));
+                    }
                     if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
                 }
             }
@@ -246,7 +317,7 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
         constexpr uint64_t DESC_HI = (uint64_t)((256u >> 4) | (1u << 14)) << 32;          // SBO 256 B, version 1
         const uint32_t lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(smem) & 0x3FFFFu) >> 4);   // LBO 128 B
         uint32_t stage = 0, phase = 0, tile_n = 0;
-        for (int64_t t = blockIdx.x; t < P.total; t += gridDim.x, ++tile_n) {
+        for (int64_t t = first; t < total2; t += step, ++tile_n) {
             ptx::mbar_wait(ACC_EMPTY, (tile_n & 1) ^ 1);
             ptx::tc_fence_after();
             for (int64_t kk = 0; kk < ks; ++kk) {
@@ -268,7 +339,8 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                             ptx::mma_i8(d, DESC_HI | a_lo, db, ID64, acc);
                         }
                     }
-                    ptx::tc_commit(EMPTY(stage));
+                    if (CL > 1) ptx::tc_commit_multicast(EMPTY(stage), (uint16_t)((1u << CL) - 1u));
+                    else ptx::tc_commit(EMPTY(stage));
                     if (kk == ks - 1) ptx::tc_commit(ACC_FULL);
                 }
                 __syncwarp();
@@ -279,44 +351,48 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
         // ===== epilogue: thread = row model (TMEM lane), loops over the 128 column models of the tile =====
         const int quad = warp & 3;
         uint32_t tile_n = 0;
-        for (int64_t t = blockIdx.x; t < P.total; t += gridDim.x, ++tile_n) {
-            int32_t I, J;
-            dg_tile_from_linear(t, P.T, I, J);
-            const int64_t i = (int64_t)I * DG_TILE + quad * 32 + lane;
+        for (int64_t t = first; t < total2; t += step, ++tile_n) {
+            int32_t SI, SJ;
+            if (CL > 1) { const int2 e = P.sched[t]; SI = e.x; SJ = e.y; } else dg_tile_from_linear(t, P.T, SI, SJ);
+            const int32_t I = CLI * SI + ri, J = CLJ * SJ + rj;
+            const bool active = I < P.T && J < P.T && I <= J;    // a cluster's block may hang over the edge / the diagonal
+            const int64_t i = (int64_t)min(I, P.T - 1) * DG_TILE + quad * 32 + lane;
             const DStat si = P.stat[i];                          // slots beyond N hold neutral records
             const double pwi = (double)si.pw * 0x1p-30;
             const int64_t rowoff = i * (2 * P.N - i - 1) / 2 - i - 1;
             ptx::mbar_wait(ACC_FULL, tile_n & 1);
             ptx::tc_fence_after();
             const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16);
+            if (active) {
 #pragma unroll 1
-            for (int c = 0; c < 8; ++c) {                        // 16-column chunks: half h = c / 4
-                const int h = c >> 2, cb = c & 3;
-                uint32_t v0[16], v1[16], v2[16];
-                ptx::tmem_ld_32x32b_x16(ta + h * HC + 16 * cb, v0);
-                if (DIGITS == 3) {
-                    ptx::tmem_ld_32x32b_x16(ta + h * HC + 64 + 16 * cb, v1);
-                    ptx::tmem_ld_32x32b_x16(ta + h * HC + 128 + 16 * cb, v2);
-                }
-                ptx::tmem_ld_wait();
-                const int64_t j0 = (int64_t)J * DG_TILE + h * DG_HALF + 16 * cb;
+                for (int c = 0; c < 8; ++c) {                    // 16-column chunks: half h = c / 4
+                    const int h = c >> 2, cb = c & 3;
+                    uint32_t v0[16], v1[16], v2[16];
+                    ptx::tmem_ld_32x32b_x16(ta + h * HC + 16 * cb, v0);
+                    if (DIGITS == 3) {
+                        ptx::tmem_ld_32x32b_x16(ta + h * HC + 64 + 16 * cb, v1);
+                        ptx::tmem_ld_32x32b_x16(ta + h * HC + 128 + 16 * cb, v2);
+                    }
+                    ptx::tmem_ld_wait();
+                    const int64_t j0 = (int64_t)J * DG_TILE + h * DG_HALF + 16 * cb;
 #pragma unroll
-                for (int e = 0; e < 16; ++e) {
-                    const int64_t j = j0 + e;
-                    if (i < P.N && j < P.N && j > i) {
-                        const DStat sj = P.stat[j];
-                        if (DIGITS == 3) {
-                            const long long dot = ((long long)(int32_t)v0[e] << 16) + ((long long)(int32_t)v1[e] << 8) +
-                                                  (long long)(int32_t)v2[e];
-                            const double res = (si.T + sj.T) - 2.0 * (double)dot * (pwi * (double)sj.pw);
-                            const float d2 = (float)(res * P.invKk);
-                            P.out[rowoff + j] = sqrtf(d2 < 0.0f ? 0.0f : d2);    // clamp (NaN stays NaN)
-                        } else {
-                            // eq. 7: S = 100 * 2 n(A and B) / (n(A) + n(B)); two empty maps are identical: 100
-                            const double den = si.T + sj.T;
-                            const double S = den > 0.0 ? __ddiv_rn(__dmul_rn(200.0, (double)(int32_t)v0[e]), den)
-                                                       : (den == 0.0 ? 100.0 : den);          // NaN model -> NaN
-                            P.out[rowoff + j] = (float)S;
+                    for (int e = 0; e < 16; ++e) {
+                        const int64_t j = j0 + e;
+                        if (i < P.N && j < P.N && j > i) {
+                            const DStat sj = P.stat[j];
+                            if (DIGITS == 3) {
+                                const long long dot = ((long long)(int32_t)v0[e] << 16) + ((long long)(int32_t)v1[e] << 8) +
+                                                      (long long)(int32_t)v2[e];
+                                const double res = (si.T + sj.T) - 2.0 * (double)dot * (pwi * (double)sj.pw);
+                                const float d2 = (float)(res * P.invKk);
+                                P.out[rowoff + j] = sqrtf(d2 < 0.0f ? 0.0f : d2);    // clamp (NaN stays NaN)
+                            } else {
+                                // eq. 7: S = 100 * 2 n(A and B) / (n(A) + n(B)); two empty maps are identical: 100
+                                const double den = si.T + sj.T;
+                                const double S = den > 0.0 ? __ddiv_rn(__dmul_rn(200.0, (double)(int32_t)v0[e]), den)
+                                                           : (den == 0.0 ? 100.0 : den);          // NaN model -> NaN
+                                P.out[rowoff + j] = (float)S;
+                            }
                         }
                     }
                 }
@@ -328,6 +404,7 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
     }
     ptx::tc_fence_before();
     __syncthreads();
+    if (CL > 1) ptx::cluster_sync();                             // no CTA leaves while a partner may still signal it
     if (warp == 1) ptx::tmem_dealloc(tmem, 512);
 }
 
@@ -344,6 +421,7 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double
     DGParams P;
     P.plane = plane;
     P.stat = stat;
+    P.sched = (const int2*)(ws + w.off_sched);
     P.out = out;
     P.N = N;
     P.ks = w.ks;
@@ -351,9 +429,43 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double
     P.total = (int64_t)P.T * (P.T + 1) / 2;
     P.invKk = 1.0 / (DG_KAPPA * DG_KAPPA * (double)w.K);
     const size_t smem = (size_t)DGCfg<DIGITS>::STAGES * DGCfg<DIGITS>::STAGE_BYTES + 8 * (2 * DGCfg<DIGITS>::STAGES + 2) + 16;
-    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(drmsd_gram_kernel<DIGITS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    // thread-block clusters with operand multicast when the matrix has enough tiles to fill the device with them
+    if (P.T >= 8) {
+        constexpr int CLI = DG_CLUSTER_I, CLJ = DG_CLUSTER_J;
+        auto kern = drmsd_gram_kernel<DIGITS, CLI, CLJ>;
+        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        cudaLaunchConfig_t cfg = {};
+        cfg.blockDim = dim3(DG_THREADS);
+        cfg.dynamicSmemBytes = smem;
+        cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = CLI * CLJ;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        cfg.gridDim = dim3((unsigned)(sms / (CLI * CLJ) * (CLI * CLJ)));
+        int clusters = 0;
+        CLUSCO_CUDA_TRY(cudaOccupancyMaxActiveClusters(&clusters, kern, &cfg));    // co-resident clusters
+        P.n_sched = dg_schedule_count(P.T, CLI, CLJ);
+        if (clusters > P.n_sched) clusters = (int)P.n_sched;
+        if (clusters >= 1) {
+            // blocks of about `clusters` super-tiles, square in tile units, so that a wave shares A rows and B columns in L2
+            int32_t bj = 1;
+            while ((int64_t)(bj + 1) * CLJ * (bj + 1) * CLJ <= (int64_t)clusters * CLI * CLJ) ++bj;
+            const int32_t bi = (bj * CLJ + CLI - 1) / CLI;
+            dg_schedule_kernel<<<1, 32, 0, s>>>(P.T, CLI, CLJ, bi, bj, (int2*)(ws + w.off_sched));
+            CLUSCO_CUDA_TRY(cudaGetLastError());
+            cfg.gridDim = dim3((unsigned)(clusters * CLI * CLJ));
+            CLUSCO_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, P));
+            return CLUSCO_OK;
+        }
+    }
+    P.n_sched = 0;
+    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(drmsd_gram_kernel<DIGITS, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t grid = P.total < sms ? P.total : sms;
-    drmsd_gram_kernel<DIGITS><<<(unsigned)grid, DG_THREADS, smem, s>>>(P);
+    drmsd_gram_kernel<DIGITS, 1, 1><<<(unsigned)grid, DG_THREADS, smem, s>>>(P);
     CLUSCO_CUDA_TRY(cudaGetLastError());
     return CLUSCO_OK;
 }

@@ -78,3 +78,15 @@ def test_cmo_full_size_sampled(clusco):
     pj = np.concatenate([pj, [1, ens.N - 1, ens.N - 1, 128, 9999]])
     want = oracle.cmo_pairs(ens.coords, 8.0, pi, pj).astype(np.float32)
     assert np.array_equal(got[wl.packed_index(pi, pj, ens.N)], want)
+
+
+@pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12)])
+def test_cmo_cluster_path_every_pair(clusco, N, L):
+    """N >= 897 takes the 2 x 2 cluster kernel with multicast operands (odd tile count: overhanging blocks)."""
+    rng = np.random.default_rng(N + L)
+    base = rng.normal(size=(1, L, 3)) * 7
+    x = (base + rng.normal(size=(N, L, 3)) * rng.uniform(0.2, 3.0, size=(N, 1, 1))).astype(np.float32)
+    want = oracle.cmo_allpairs(x, 9.0).astype(np.float32)
+    got = clusco.clusco_cmo_allpairs(_dev(x), 9.0).cpu().numpy()
+    assert np.array_equal(got, want)
+    assert want.min() < 90.0

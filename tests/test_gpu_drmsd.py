@@ -98,3 +98,15 @@ def test_drmsd_full_size_sampled(clusco):
     pj = np.concatenate([pj, [1, ens.N - 1, ens.N - 1, 128, 9999]])
     d_ref, d2_ref = oracle.drmsd_pairs(ens.coords, pi, pj)
     _check(got[wl.packed_index(pi, pj, ens.N)], d_ref, d2_ref, "C3 sampled")
+
+
+@pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12)])
+def test_drmsd_cluster_path_every_pair(clusco, N, L):
+    """N >= 897 (8 tiles per side) takes the 2 x 2 cluster kernel with multicast operands; T = 9 is odd, so the
+    last cluster row / column hangs over the edge and the diagonal blocks hold one masked tile."""
+    rng = np.random.default_rng(N + L)
+    base = rng.normal(size=(1, L, 3)) * 7
+    x = (base + rng.normal(size=(N, L, 3)) * rng.uniform(0.2, 3.0, size=(N, 1, 1))).astype(np.float32)
+    d_ref, d2_ref = oracle.drmsd_allpairs(x)
+    got = clusco.clusco_drmsd_allpairs(_dev(x)).cpu().numpy()
+    _check(got, d_ref, d2_ref, f"cluster N={N} L={L}")
