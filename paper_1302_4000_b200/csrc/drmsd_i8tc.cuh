@@ -121,6 +121,15 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
     const bool in_range = dmax < 1.0e9;
     ex = max(-30, min(30, ex));
     const double scale = ldexp(DG_KAPPA, 23 - ex);
+    // CMO: sqrt(s) < cutoff  <=>  s < s_star, s_star = the smallest double whose correctly rounded square root is
+    // >= cutoff (the rounded square root is monotone), found once per thread by stepping from cutoff^2: the
+    // per-entry decision needs no square root and stays bit-identical to eq. 6 evaluated literally in FP64
+    double s_star = 0.0;
+    if (DIGITS == 1) {
+        s_star = __dmul_rn(cutoff, cutoff);
+        for (int it = 0; it < 8 && s_star > 0.0 && sqrt(s_star) >= cutoff; ++it) s_star = nextafter(s_star, 0.0);
+        for (int it = 0; it < 8 && sqrt(s_star) < cutoff; ++it) s_star = nextafter(s_star, 1.0e300);
+    }
     // pass 2: integers, digits, plane bytes
     const int64_t t64 = n >> 6;
     const int g = (int)(n & 63) >> 3, r8 = (int)(n & 7);
@@ -133,8 +142,17 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         int I = 0;
         if (valid && k < K) {
             while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
-            const double d = sqrt(dist2(i, i + 1 + pos));
-            I = DIGITS == 3 ? __double2int_rn(d * scale) : (d < cutoff ? 1 : 0);
+            const double s2 = dist2(i, i + 1 + pos);
+            if (DIGITS == 3) {
+                // sqrt by the fp32 reciprocal square root + one FP64 Newton step: relative error ~1e-13, far below the
+                // 2^-24 quantisation step (the IEEE double square root is ~40 instructions, this is 5)
+                const double rf = (double)rsqrtf((float)s2);
+                const double d0 = s2 * rf;
+                const double d = s2 > 0.0 ? fma(0.5 * rf, fma(-d0, d0, s2), d0) : 0.0;
+                I = __double2int_rn(d * scale);
+            } else {
+                I = s2 < s_star ? 1 : 0;
+            }
             pos += 32;
         }
         if (DIGITS == 1) {
@@ -203,16 +221,27 @@ __host__ __device__ __forceinline__ bool dg_super_valid(int32_t SI, int32_t SJ, 
 }
 __global__ void dg_schedule_kernel(int32_t T, int32_t cli, int32_t clj, int32_t bi, int32_t bj, int2* __restrict__ sched)
 {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    // one warp: 32 candidates (block-major order) per round, compacted with a ballot
+    if (blockIdx.x != 0 || threadIdx.x >= 32) return;
+    const int lane = threadIdx.x;
     const int32_t TI = (T + cli - 1) / cli, TJ = (T + clj - 1) / clj;
+    const int32_t NBI = (TI + bi - 1) / bi, NBJ = (TJ + bj - 1) / bj;
+    const int64_t per_block = (int64_t)bi * bj, total = (int64_t)NBI * NBJ * per_block;
     int64_t n = 0;
-    for (int32_t BI = 0; BI * bi < TI; ++BI)
-        for (int32_t BJ = 0; BJ * bj < TJ; ++BJ)
-            for (int32_t si = 0; si < bi; ++si)
-                for (int32_t sj = 0; sj < bj; ++sj) {
-                    const int32_t SI = BI * bi + si, SJ = BJ * bj + sj;
-                    if (SI < TI && SJ < TJ && dg_super_valid(SI, SJ, cli, clj, T)) sched[n++] = make_int2(SI, SJ);
-                }
+    for (int64_t c0 = 0; c0 < total; c0 += 32) {
+        const int64_t c = c0 + lane;
+        bool ok = false;
+        int32_t SI = 0, SJ = 0;
+        if (c < total) {
+            const int64_t blk = c / per_block, in = c - blk * per_block;
+            SI = (int32_t)(blk / NBJ) * bi + (int32_t)(in / bj);
+            SJ = (int32_t)(blk % NBJ) * bj + (int32_t)(in % bj);
+            ok = SI < TI && SJ < TJ && dg_super_valid(SI, SJ, cli, clj, T);
+        }
+        const uint32_t m = __ballot_sync(0xffffffffu, ok);
+        if (ok) sched[n + __popc(m & ((1u << lane) - 1u))] = make_int2(SI, SJ);
+        n += __popc(m);
+    }
 }
 static inline int64_t dg_schedule_count(int32_t T, int32_t cli, int32_t clj)
 {
