@@ -356,17 +356,18 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                     const uint32_t a_lo = lo0 + stage * (DG_STAGE_BYTES >> 4);
                     const uint32_t b_lo = a_lo + ((2 * DIGITS * DG_SLAB) >> 4);
                     const uint32_t acc = kk > 0;
+                    if (DIGITS == 3) {
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const uint64_t db = DESC_HI | (b_lo + h * ((DIGITS * DG_SLAB) >> 4));
-                        const uint32_t d = tmem + h * HC;
-                        if (DIGITS == 3) {
+                        for (int h = 0; h < 2; ++h) {
+                            const uint64_t db = DESC_HI | (b_lo + h * ((DIGITS * DG_SLAB) >> 4));
+                            const uint32_t d = tmem + h * HC;
                             ptx::mma_i8(d, DESC_HI | a_lo, db, ID192, acc);
                             ptx::mma_i8(d + 64, DESC_HI | (a_lo + ((2 * DG_SLAB) >> 4)), db, ID128, 1);
                             ptx::mma_i8(d + 128, DESC_HI | (a_lo + ((4 * DG_SLAB) >> 4)), db, ID64, 1);
-                        } else {
-                            ptx::mma_i8(d, DESC_HI | a_lo, db, ID64, acc);
                         }
+                    } else {
+                        // one digit: the two 64-row B halves are contiguous in the stage, so ONE N = 128 MMA covers the tile
+                        ptx::mma_i8(tmem, DESC_HI | a_lo, DESC_HI | b_lo, ID128, acc);
                     }
                     if (CL > 1) ptx::tc_commit_multicast(EMPTY(stage), (uint16_t)((1u << CL) - 1u));
                     else ptx::tc_commit(EMPTY(stage));
