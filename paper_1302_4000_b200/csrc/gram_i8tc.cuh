@@ -38,6 +38,8 @@ constexpr int I8_ACC_BUFS = 2;
 constexpr int I8_A_TMEM_COL = I8_ACC_BUFS * I8_ACC_COLS;   // the A tile lives in TMEM columns 288 .. 288 + 24 ksteps
 constexpr int I8_EPI_WARPS = 16;
 constexpr int I8_THREADS = (2 + I8_EPI_WARPS) * 32;
+constexpr int I8_HIT_CAP = 64;                 // BELOW: hits staged per epilogue warp before one atomic reserves their slots
+constexpr size_t I8_HIT_BYTES = (size_t)I8_EPI_WARPS * I8_HIT_CAP * 12;
 
 static inline bool i8tc_supported(int32_t L) { return L >= 1 && L <= 32 * I8_MAX_KSTEPS; }
 
@@ -373,6 +375,30 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         // ROWSTATS: running sum / count of the row this lane group is on (rows persist over consecutive tiles)
         double acc_sum = 0.0;
         int32_t acc_cnt = 0, acc_i = -1;
+        // BELOW: hits are staged per warp in shared memory and appended I8_HIT_CAP at a time -- ONE atomic on the shared
+        // counter per flush (a single hot address serialises in L2: one atomic per warp and tile cost +30 % at C3)
+        uint8_t* hit_base = reinterpret_cast<uint8_t*>(tmem_slot) + 16 + (size_t)ew * I8_HIT_CAP * 12;
+        int32_t* hit_i = reinterpret_cast<int32_t*>(hit_base);
+        int32_t* hit_j = hit_i + I8_HIT_CAP;
+        float* hit_c = reinterpret_cast<float*>(hit_j + I8_HIT_CAP);
+        int nhit = 0;                                            // warp-uniform
+        auto flush_hits = [&]() {
+            if (nhit == 0) return;
+            __syncwarp();
+            unsigned long long base = 0ull;
+            if (lane == 0) base = atomicAdd(P.sink.count, (unsigned long long)nhit);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            for (int e = lane; e < nhit; e += 32) {
+                const int64_t slot = (int64_t)base + e;
+                if (slot < P.sink.capacity) {
+                    P.sink.pair_i[slot] = hit_i[e];
+                    P.sink.pair_j[slot] = hit_j[e];
+                    P.sink.pair_c[slot] = hit_c[e];
+                }
+            }
+            __syncwarp();
+            nhit = 0;
+        };
         auto flush_row = [&]() {
             if (c4 == 0 && acc_i >= 0 && acc_i < (int32_t)P.N) {
                 atomicAdd(P.sink.rowsum + acc_i, acc_sum);
@@ -391,30 +417,21 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 if (pend.ok0) pend.dst[0] = c.x;
                 if (pend.ok1) pend.dst[4] = c.y;
             } else if (MODE == SINK_BELOW) {
-                // warp-aggregated append: one atomic on the shared counter per warp and tile
                 const bool h0 = pend.ok0 && c.x < P.sink.cutoff, h1 = pend.ok1 && c.y < P.sink.cutoff;
                 const uint32_t m0 = __ballot_sync(0xffffffffu, h0), m1 = __ballot_sync(0xffffffffu, h1);
-                if (m0 | m1) {
-                    unsigned long long base = 0ull;
-                    if (lane == 0) base = atomicAdd(P.sink.count, (unsigned long long)(__popc(m0) + __popc(m1)));
-                    base = __shfl_sync(0xffffffffu, base, 0);
+                const int add = __popc(m0) + __popc(m1);
+                if (add) {
+                    if (nhit + add > I8_HIT_CAP) flush_hits();
                     const uint32_t lt = (1u << lane) - 1u;
                     if (h0) {
-                        const int64_t slot = (int64_t)base + __popc(m0 & lt);
-                        if (slot < P.sink.capacity) {
-                            P.sink.pair_i[slot] = pend.i;
-                            P.sink.pair_j[slot] = pend.j0;
-                            P.sink.pair_c[slot] = c.x;
-                        }
+                        const int e = nhit + __popc(m0 & lt);
+                        hit_i[e] = pend.i; hit_j[e] = pend.j0; hit_c[e] = c.x;
                     }
                     if (h1) {
-                        const int64_t slot = (int64_t)base + __popc(m0) + __popc(m1 & lt);
-                        if (slot < P.sink.capacity) {
-                            P.sink.pair_i[slot] = pend.i;
-                            P.sink.pair_j[slot] = pend.j0 + 4;
-                            P.sink.pair_c[slot] = c.y;
-                        }
+                        const int e = nhit + __popc(m0) + __popc(m1 & lt);
+                        hit_i[e] = pend.i; hit_j[e] = pend.j0 + 4; hit_c[e] = c.y;
                     }
+                    nhit += add;
                 }
             } else {
                 // the warp holds 8 rows (r) x 8 columns (c4, c4 + 4): reduce over the columns for the row sums
@@ -543,6 +560,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         }
         if (have_pend) finish_pending();
         if (MODE == SINK_ROWSTATS) flush_row();
+        if (MODE == SINK_BELOW) flush_hits();
     }
     ptx::tc_fence_before();
     __syncthreads();
@@ -553,10 +571,10 @@ static inline size_t i8tc_smem_bytes(int ks, int stages)
 {
     return (size_t)3 * ks * I8_A_SLAB + (size_t)stages * ks * I8_B_SLAB + 8 * (2 * stages + 2 + 2 * I8_ACC_BUFS) + 16;
 }
-static inline int i8tc_stages(int ks)
+static inline int i8tc_stages(int ks, size_t extra)
 {
     int st = I8_MAX_STAGES;
-    while (st > 2 && i8tc_smem_bytes(ks, st) > 227 * 1024) --st;
+    while (st > 2 && i8tc_smem_bytes(ks, st) + extra > 227 * 1024) --st;
     return st;
 }
 
@@ -594,8 +612,9 @@ static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t 
     P.tiles.I_hi = (row_end + I8_ROW_MODELS - 1) / I8_ROW_MODELS;
     P.tiles.total = i8_tiles_before(P.tiles, P.tiles.I_hi);
     if (P.tiles.total <= 0) return CLUSCO_OK;
-    P.stages = i8tc_stages(ks);
-    const size_t smem = i8tc_smem_bytes(ks, P.stages);
+    const size_t extra = MODE == SINK_BELOW ? I8_HIT_BYTES + 16 : 0;       // per-warp hit staging after the barriers
+    P.stages = i8tc_stages(ks, extra);
+    const size_t smem = i8tc_smem_bytes(ks, P.stages) + extra;
     const int64_t grid = P.tiles.total < sms ? P.tiles.total : sms;
     switch (ks) {
 #define I8_LAUNCH(KS)                                                                                                  \
