@@ -11,14 +11,16 @@
 // six int8 products accumulated EXACTLY in int32 TMEM accumulators (|V| <= 3 K 2^14 < 2^31 needs L <= 296), and
 // |d|^2 is taken from the same integers (exact in 64 bits), so quantisation cancels for similar models.
 //
-// Operand plane (one, shared by both operands): P[tile64][k-step][digit][2048 B] -- for 64 consecutive models and 32
+// Operand plane (one, shared by both operands): P[tile][k-step][digit][4096 B] -- for 128 consecutive models and 32
 // consecutive entries of K, the int8 digit `digit` as a shared-memory image in tcgen05's canonical K-major no-swizzle
-// core-matrix layout (8 row groups x [2 x 128 B]), fetched by plain 1-D bulk copies.
+// core-matrix layout (16 row groups x [2 x 128 B]).  Consecutive k-steps of a tile are contiguous, so the A (or B)
+// operand of a stage of KG k-steps is ONE contiguous run fetched by ONE 1-D bulk copy (the per-copy / per-stage
+// handshake, not the bytes, was what limited an earlier layout with eight 2 KB pieces per k-step).
 //
-// Kernel: persistent, one CTA per SM, tile = 128 x 128 models (two 64-column halves), warp 0 = bulk-copy producer
-// (ring of 24 KB stages: A = 3 digits x 128 rows, B = 2 halves x 3 digits x 64 rows), warp 1 = MMA issuer (six MMAs
-// per k-step: A(g0).[B(g0);B(g1);B(g2)]^T, A(g1).[B(g0);B(g1)]^T, A(g2).B(g0)^T for each half, N = 192/128/64),
-// warps 2..5 = epilogue (FP64: the K loop is ~1000 k-steps long, the epilogue is <1 % of a tile).
+// Kernel: persistent, one CTA per SM, tile = 128 x 128 models, warp 0 = bulk-copy producer (ring of stages of KG
+// k-steps: A and B, each KG x DIGITS x 4 KB), warp 1 = MMA issuer -- per k-step six N = 128 MMAs, level v (TMEM columns
+// 128 v ...) collecting the digit products A(ga).B(gb)^T with ga + gb = v -- warps 2..5 = epilogue (FP64: the K loop
+// is ~1000 k-steps long, the epilogue is <1 % of a tile).  2 x 2 thread-block clusters multicast the operands (below).
 #pragma once
 #include "common.cuh"
 #include "prep.cuh"
@@ -28,19 +30,23 @@ namespace clusco {
 
 constexpr double DG_KAPPA = 127.0 / 128.0;
 constexpr int DG_MAX_L = 296;                  // 3 K 2^14 < 2^31 with K = L(L-1)/2
-constexpr int DG_TILE = 128, DG_HALF = 64;
-constexpr int DG_SLAB = 2048;                  // bytes of one (tile64, k-step, digit) image: 64 rows x 32 entries
+constexpr int DG_TILE = 128;
+constexpr int DG_SLAB = 4096;                  // bytes of one (tile, k-step, digit) image: 128 rows x 32 entries
 // DIGITS = 3: dRMSD (24-bit fixed-point distances); DIGITS = 1: CMO (0/1 contact maps, eq. 6-7) on the same kernels
+#ifndef DG_KG3
+#define DG_KG3 2                               // dRMSD: k-steps per stage (measured Gram time at C3's shape: 1 -> 7.11 ms, 2 -> 6.73 ms)
+#endif
 template <int DIGITS> struct DGCfg {
-    static constexpr int STAGE_BYTES = DIGITS * 2 * DG_SLAB + 2 * DIGITS * DG_SLAB;   // A (digits x 128 rows) + B (2 halves x digits x 64)
-    static constexpr int STAGES = DIGITS == 3 ? 8 : 24;
-    static constexpr int HALF_COLS = 64 * DIGITS;                                      // TMEM columns per 64-model half
+    static constexpr int KG = DIGITS == 3 ? DG_KG3 : 4;                 // k-steps per stage (consecutive k-steps are contiguous)
+    static constexpr int OPER_BYTES = KG * DIGITS * DG_SLAB;            // one operand (A or B tile) of a stage: ONE contiguous run
+    static constexpr int STAGE_BYTES = 2 * OPER_BYTES;
+    static constexpr int STAGES = (216 * 1024) / STAGE_BYTES;
 };
 constexpr int DG_THREADS = 6 * 32;
 constexpr int DG_PREP_WARPS = 8;
 #ifndef DG_CLUSTER_I
 #define DG_CLUSTER_I 2                         // cluster shape of the Gram kernel: CLI tile rows x CLJ tile columns
-#define DG_CLUSTER_J 2                         // (measured at C3's shape: 2x2 7.46 ms, 1x2 7.78 ms, 2x1 9.25 ms, none 8.24 ms)
+#define DG_CLUSTER_J 2                         // (measured at C3's shape with KG = 2: 2x2 6.73 ms, 1x2 6.97 ms)
 #endif
 
 struct __align__(16) DStat {
@@ -50,7 +56,7 @@ struct __align__(16) DStat {
 };
 
 struct DWorkspace {
-    int64_t N, Np, K, ks, tiles64;
+    int64_t N, Np, K, ks, tiles;        // ks = k-steps, padded to a multiple of the stage's k-group
     size_t off_stat, off_sched, off_plane, total;
 };
 static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L, int digits = 3)
@@ -59,8 +65,9 @@ static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L, int digits
     w.N = N;
     w.Np = round_up(N, DG_TILE);
     w.K = (int64_t)L * (L - 1) / 2;
-    w.ks = (w.K + 31) / 32;
-    w.tiles64 = w.Np / DG_HALF;
+    const int64_t kg = digits == 3 ? DGCfg<3>::KG : DGCfg<1>::KG;
+    w.ks = round_up((w.K + 31) / 32, kg);
+    w.tiles = w.Np / DG_TILE;
     size_t o = 0;
     w.off_stat = o;
     o += (size_t)round_up((int64_t)sizeof(DStat) * w.Np, 256);
@@ -70,7 +77,7 @@ static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L, int digits
         o += (size_t)round_up((int64_t)sizeof(int2) * (T * (T + 1) / 2 + T), 256);
     }
     w.off_plane = o;
-    o += (size_t)round_up(w.tiles64 * w.ks * digits * DG_SLAB, 256);
+    o += (size_t)round_up(w.tiles * w.ks * digits * DG_SLAB, 256);
     w.total = o + 256;
     return w;
 }
@@ -131,10 +138,10 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         for (int it = 0; it < 8 && sqrt(s_star) < cutoff; ++it) s_star = nextafter(s_star, 1.0e300);
     }
     // pass 2: integers, digits, plane bytes
-    const int64_t t64 = n >> 6;
-    const int g = (int)(n & 63) >> 3, r8 = (int)(n & 7);
+    const int64_t t128 = n >> 7;
+    const int g = (int)(n & 127) >> 3, r8 = (int)(n & 7);
     const int kc = lane >> 4, kb = lane & 15;
-    int8_t* base = plane + (t64 * ks * DIGITS) * DG_SLAB + g * 256 + kc * 128 + r8 * 16 + kb;
+    int8_t* base = plane + (t128 * ks * DIGITS) * DG_SLAB + g * 256 + kc * 128 + r8 * 16 + kb;
     long long sumsq = 0ll;
     int i = 0, pos = lane;
     for (int64_t kk = 0; kk < ks; ++kk) {
@@ -262,7 +269,7 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
 {
     constexpr int CL = CLI * CLJ;                                // CTAs per cluster: CLI tile rows x CLJ tile columns
     constexpr int DG_STAGES = DGCfg<DIGITS>::STAGES, DG_STAGE_BYTES = DGCfg<DIGITS>::STAGE_BYTES;
-    constexpr int HC = DGCfg<DIGITS>::HALF_COLS;
+    constexpr int KG = DGCfg<DIGITS>::KG, OPER = DGCfg<DIGITS>::OPER_BYTES;
     extern __shared__ __align__(128) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)DG_STAGES * DG_STAGE_BYTES);
     const uint32_t bar0 = ptx::smem_u32(bars);
@@ -289,7 +296,7 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
     if (CL > 1) ptx::cluster_sync();                             // every CTA's barriers exist before any remote signal
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    const int64_t ks = P.ks;
+    const int64_t ng = P.ks / KG;                                // stages per tile (k-groups)
     // CL == 1: tiles I <= J row-major (dg_tile_from_linear); CL > 1: the super-tile list written by dg_schedule_kernel
     const int64_t total2 = CL > 1 ? P.n_sched : P.total;
     const int64_t first = blockIdx.x / CL, step = gridDim.x / CL;
@@ -298,80 +305,68 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
         // ===== producer =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
-            const int64_t t64_stride = ks * DIGITS * DG_SLAB;
+            const int64_t tile_stride = P.ks * DIGITS * DG_SLAB;
             for (int64_t t = first; t < total2; t += step) {
                 int32_t SI, SJ;
                 if (CL > 1) { const int2 e = P.sched[t]; SI = e.x; SJ = e.y; } else dg_tile_from_linear(t, P.T, SI, SJ);
                 const int32_t I = min(CLI * SI + ri, P.T - 1), J = min(CLJ * SJ + rj, P.T - 1);   // clamped: results are masked
-                const int8_t* a0 = P.plane + (int64_t)(2 * I) * t64_stride;               // tile64 2I; 2I + 1 follows
-                const int8_t* b0 = P.plane + (int64_t)(2 * J) * t64_stride;
-                for (int64_t kk = 0; kk < ks; ++kk) {
+                const int8_t* a0 = P.plane + (int64_t)I * tile_stride;
+                const int8_t* b0 = P.plane + (int64_t)J * tile_stride;
+                for (int64_t kg = 0; kg < ng; ++kg) {
                     ptx::mbar_wait(EMPTY(stage), phase ^ 1);
                     ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
                     const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
-                    const uint32_t sB = sA + 2 * DIGITS * DG_SLAB;
-                    // A tile: needed by the CLJ CTAs of my tile row -- with CLJ == 2 I fetch half rj and multicast it
-                    if (CLJ == 2) {
-                        const uint16_t row_mask = (uint16_t)(3u << (ri * CLJ));
-#pragma unroll
-                        for (int d = 0; d < DIGITS; ++d)
-                            ptx::bulk_g2s_multicast(sA + (2 * d + rj) * DG_SLAB, a0 + rj * t64_stride + (kk * DIGITS + d) * DG_SLAB,
-                                                    DG_SLAB, FULL(stage), row_mask);
-                    } else {
-#pragma unroll
-                        for (int d = 0; d < DIGITS; ++d)
-#pragma unroll
-                            for (int h = 0; h < 2; ++h)
-                                ptx::bulk_g2s(sA + (2 * d + h) * DG_SLAB, a0 + h * t64_stride + (kk * DIGITS + d) * DG_SLAB,
-                                              DG_SLAB, FULL(stage));
-                    }
-                    // B tile: needed by the CLI CTAs of my tile column -- with CLI == 2 I fetch half ri and multicast it
-                    if (CLI == 2) {
-                        const uint16_t col_mask = (uint16_t)((1u | (1u << CLJ)) << rj);
-                        ptx::bulk_g2s_multicast(sB + ri * DIGITS * DG_SLAB, b0 + ri * t64_stride + kk * DIGITS * DG_SLAB,
-                                                DIGITS * DG_SLAB, FULL(stage), col_mask);
-                    } else {
-#pragma unroll
-                        for (int h = 0; h < 2; ++h)
-                            ptx::bulk_g2s(sB + h * DIGITS * DG_SLAB, b0 + h * t64_stride + kk * DIGITS * DG_SLAB,
-                                          DIGITS * DG_SLAB, FULL(stage));
-                    }
+                    const uint32_t sB = sA + OPER;
+                    // a stage's A (and B) operand is one contiguous run of the plane: KG k-steps x DIGITS slabs.
+                    // A is needed by the CLJ CTAs of my tile row: with CLJ == 2 I fetch half rj of the run and multicast it
+                    if (CLJ == 2)
+                        ptx::bulk_g2s_multicast(sA + rj * (OPER / 2), a0 + kg * OPER + rj * (OPER / 2), OPER / 2, FULL(stage),
+                                                (uint16_t)(3u << (ri * CLJ)));
+                    else
+                        ptx::bulk_g2s(sA, a0 + kg * OPER, OPER, FULL(stage));
+                    // B is needed by the CLI CTAs of my tile column: with CLI == 2 I fetch half ri and multicast it
+                    if (CLI == 2)
+                        ptx::bulk_g2s_multicast(sB + ri * (OPER / 2), b0 + kg * OPER + ri * (OPER / 2), OPER / 2, FULL(stage),
+                                                (uint16_t)((1u | (1u << CLJ)) << rj));
+                    else
+                        ptx::bulk_g2s(sB, b0 + kg * OPER, OPER, FULL(stage));
                     if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
                 }
             }
         }
     } else if (warp == 1) {
         // ===== MMA issuer (warp-uniform loop, one elected lane issues) =====
-        constexpr uint32_t ID192 = ptx::idesc_s8(128, 192), ID128 = ptx::idesc_s8(128, 128), ID64 = ptx::idesc_s8(128, 64);
+        constexpr uint32_t ID128 = ptx::idesc_s8(128, 128);
         constexpr uint64_t DESC_HI = (uint64_t)((256u >> 4) | (1u << 14)) << 32;          // SBO 256 B, version 1
         const uint32_t lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(smem) & 0x3FFFFu) >> 4);   // LBO 128 B
         uint32_t stage = 0, phase = 0, tile_n = 0;
         for (int64_t t = first; t < total2; t += step, ++tile_n) {
             ptx::mbar_wait(ACC_EMPTY, (tile_n & 1) ^ 1);
             ptx::tc_fence_after();
-            for (int64_t kk = 0; kk < ks; ++kk) {
+            for (int64_t kg = 0; kg < ng; ++kg) {
                 ptx::mbar_wait(FULL(stage), phase);
                 ptx::tc_fence_after();
                 if (ptx::elect_one()) {
                     const uint32_t a_lo = lo0 + stage * (DG_STAGE_BYTES >> 4);
-                    const uint32_t b_lo = a_lo + ((2 * DIGITS * DG_SLAB) >> 4);
-                    const uint32_t acc = kk > 0;
-                    if (DIGITS == 3) {
+                    const uint32_t b_lo = a_lo + (OPER >> 4);
+                    constexpr uint32_t SL = DG_SLAB >> 4;
 #pragma unroll
-                        for (int h = 0; h < 2; ++h) {
-                            const uint64_t db = DESC_HI | (b_lo + h * ((DIGITS * DG_SLAB) >> 4));
-                            const uint32_t d = tmem + h * HC;
-                            ptx::mma_i8(d, DESC_HI | a_lo, db, ID192, acc);
-                            ptx::mma_i8(d + 64, DESC_HI | (a_lo + ((2 * DG_SLAB) >> 4)), db, ID128, 1);
-                            ptx::mma_i8(d + 128, DESC_HI | (a_lo + ((4 * DG_SLAB) >> 4)), db, ID64, 1);
+                    for (int q = 0; q < KG; ++q) {
+                        const uint32_t acc = (kg > 0 || q > 0) ? 1u : 0u;
+                        const uint32_t aq = a_lo + q * DIGITS * SL, bq = b_lo + q * DIGITS * SL;
+                        // level v (TMEM columns 128 v ...) collects the digit products A(ga) . B(gb)^T with ga + gb = v
+                        ptx::mma_i8(tmem, DESC_HI | aq, DESC_HI | bq, ID128, acc);
+                        if (DIGITS == 3) {
+                            ptx::mma_i8(tmem + 128, DESC_HI | aq, DESC_HI | (bq + SL), ID128, acc);
+                            ptx::mma_i8(tmem + 128, DESC_HI | (aq + SL), DESC_HI | bq, ID128, 1);
+                            ptx::mma_i8(tmem + 256, DESC_HI | aq, DESC_HI | (bq + 2 * SL), ID128, acc);
+                            ptx::mma_i8(tmem + 256, DESC_HI | (aq + SL), DESC_HI | (bq + SL), ID128, 1);
+                            ptx::mma_i8(tmem + 256, DESC_HI | (aq + 2 * SL), DESC_HI | bq, ID128, 1);
                         }
-                    } else {
-                        // one digit: the two 64-row B halves are contiguous in the stage, so ONE N = 128 MMA covers the tile
-                        ptx::mma_i8(tmem, DESC_HI | a_lo, DESC_HI | b_lo, ID128, acc);
                     }
                     if (CL > 1) ptx::tc_commit_multicast(EMPTY(stage), (uint16_t)((1u << CL) - 1u));
                     else ptx::tc_commit(EMPTY(stage));
-                    if (kk == ks - 1) ptx::tc_commit(ACC_FULL);
+                    if (kg == ng - 1) ptx::tc_commit(ACC_FULL);
                 }
                 __syncwarp();
                 if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
@@ -395,16 +390,15 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
             const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16);
             if (active) {
 #pragma unroll 1
-                for (int c = 0; c < 8; ++c) {                    // 16-column chunks: half h = c / 4
-                    const int h = c >> 2, cb = c & 3;
+                for (int c = 0; c < 8; ++c) {                    // 16-column chunks of the 128 column models
                     uint32_t v0[16], v1[16], v2[16];
-                    ptx::tmem_ld_32x32b_x16(ta + h * HC + 16 * cb, v0);
+                    ptx::tmem_ld_32x32b_x16(ta + 16 * c, v0);
                     if (DIGITS == 3) {
-                        ptx::tmem_ld_32x32b_x16(ta + h * HC + 64 + 16 * cb, v1);
-                        ptx::tmem_ld_32x32b_x16(ta + h * HC + 128 + 16 * cb, v2);
+                        ptx::tmem_ld_32x32b_x16(ta + 128 + 16 * c, v1);
+                        ptx::tmem_ld_32x32b_x16(ta + 256 + 16 * c, v2);
                     }
                     ptx::tmem_ld_wait();
-                    const int64_t j0 = (int64_t)J * DG_TILE + h * DG_HALF + 16 * cb;
+                    const int64_t j0 = (int64_t)J * DG_TILE + 16 * c;
 #pragma unroll
                     for (int e = 0; e < 16; ++e) {
                         const int64_t j = j0 + e;
