@@ -110,20 +110,23 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         const double dz = (double)x[3 * i + 2] - (double)x[3 * j + 2];
         return __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
     };
-    // pass 1: largest distance -> power-of-two scale with dmax 2^-ex in [0.5, 1)
+    // scale: a power of two 2^ex with dmax 2^-ex < 1, from the bound  amax <= dmax <= 2 amax,  amax = the largest
+    // distance of an atom from the centroid (the centroid lies in the convex hull, so some atom is at least amax away
+    // from the farthest one): at most one bit of the 24 is given up, and no pass over the K distances is needed
     double m2 = 0.0;
     if (valid && DIGITS == 3) {
-        int i = 0, pos = lane;                                   // entry k = lane, lane + 32, ...: pair (i, i + 1 + pos)
-        for (int64_t k = lane; k < K; k += 32) {
-            while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
-            m2 = fmax(m2, dist2(i, i + 1 + pos));
-            pos += 32;
+        double c0 = 0.0, c1 = 0.0, c2 = 0.0;
+        for (int a = lane; a < L; a += 32) { c0 += (double)x[3 * a]; c1 += (double)x[3 * a + 1]; c2 += (double)x[3 * a + 2]; }
+        c0 = warp_sum(c0) / (double)L; c1 = warp_sum(c1) / (double)L; c2 = warp_sum(c2) / (double)L;
+        for (int a = lane; a < L; a += 32) {
+            const double dx = (double)x[3 * a] - c0, dy = (double)x[3 * a + 1] - c1, dz = (double)x[3 * a + 2] - c2;
+            m2 = fmax(m2, dx * dx + dy * dy + dz * dz);
         }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) m2 = fmax(m2, __shfl_xor_sync(0xffffffffu, m2, o));
     int ex = 0;
-    const double dmax = sqrt(m2);
+    const double dmax = 2.0 * sqrt(m2);
     if (dmax > 0.0 && dmax < 1.0e30) (void)frexp(dmax, &ex);
     const bool in_range = dmax < 1.0e9;
     ex = max(-30, min(30, ex));
@@ -137,47 +140,61 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         for (int it = 0; it < 8 && s_star > 0.0 && sqrt(s_star) >= cutoff; ++it) s_star = nextafter(s_star, 0.0);
         for (int it = 0; it < 8 && sqrt(s_star) < cutoff; ++it) s_star = nextafter(s_star, 1.0e300);
     }
-    // pass 2: integers, digits, plane bytes
+    // one pass over the K entries: a warp covers 4 k-steps per trip, lane = (k-step sub, group j8 of 4 consecutive
+    // entries), so that the digit bytes of 4 entries leave as one 32-bit store per digit
     const int64_t t128 = n >> 7;
     const int g = (int)(n & 127) >> 3, r8 = (int)(n & 7);
-    const int kc = lane >> 4, kb = lane & 15;
-    int8_t* base = plane + (t128 * ks * DIGITS) * DG_SLAB + g * 256 + kc * 128 + r8 * 16 + kb;
+    const int sub = lane >> 3, j8 = lane & 7;
+    int8_t* base = plane + (t128 * ks * DIGITS) * DG_SLAB + g * 256 + (j8 >> 2) * 128 + r8 * 16 + (j8 & 3) * 4;
     long long sumsq = 0ll;
-    int i = 0, pos = lane;
-    for (int64_t kk = 0; kk < ks; ++kk) {
-        const int64_t k = kk * 32 + lane;
-        int I = 0;
-        if (valid && k < K) {
+    int i = 0, pos = sub * 32 + 4 * j8;                          // entry k = (4 trip + sub) 32 + 4 j8: pair (i, i + 1 + pos)
+    for (int64_t kk0 = 0; kk0 < ks; kk0 += 4) {
+        const int64_t kk = kk0 + sub;
+        const int64_t k0 = kk * 32 + 4 * j8;
+        uint32_t w0 = 0u, w1 = 0u, w2 = 0u;
+        if (valid && k0 < K) {
             while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
-            const double s2 = dist2(i, i + 1 + pos);
-            if (DIGITS == 3) {
-                // sqrt by the fp32 reciprocal square root + one FP64 Newton step: relative error ~1e-13, far below the
-                // 2^-24 quantisation step (the IEEE double square root is ~40 instructions, this is 5)
-                const double rf = (double)rsqrtf((float)s2);
-                const double d0 = s2 * rf;
-                const double d = s2 > 0.0 ? fma(0.5 * rf, fma(-d0, d0, s2), d0) : 0.0;
-                I = __double2int_rn(d * scale);
-            } else {
-                I = s2 < s_star ? 1 : 0;
+            int ii = i, pp = pos;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                if (k0 + e < K) {
+                    if (pp >= L - 1 - ii) { pp -= L - 1 - ii; ++ii; }     // at most one row wrap per step (rows are non-empty here)
+                    const double s2 = dist2(ii, ii + 1 + pp);
+                    ++pp;
+                    if (DIGITS == 3) {
+                        // sqrt by the fp32 reciprocal square root + one FP64 Newton step: relative error ~1e-13, far
+                        // below the 2^-24 quantisation step (the IEEE double square root is ~40 instructions)
+                        const double rf = (double)rsqrtf((float)s2);
+                        const double d0 = s2 * rf;
+                        const double d = s2 > 0.0 ? fma(0.5 * rf, fma(-d0, d0, s2), d0) : 0.0;
+                        const int I = __double2int_rn(d * scale);
+                        const int g2 = (int)(int8_t)(I & 0xff);
+                        const int I1 = (I - g2) >> 8;
+                        const int g1 = (int)(int8_t)(I1 & 0xff);
+                        const int g0 = (I1 - g1) >> 8;
+                        // |d|^2 from the SAME three levels the Gram keeps (I^2 minus the two dropped low-order levels),
+                        // so that an identical pair cancels to exactly 0
+                        sumsq += (long long)I * (long long)I - (long long)(512 * g1 * g2 + g2 * g2);
+                        w0 |= (uint32_t)(g0 & 0xff) << (8 * e);
+                        w1 |= (uint32_t)(g1 & 0xff) << (8 * e);
+                        w2 |= (uint32_t)(g2 & 0xff) << (8 * e);
+                    } else {
+                        const uint32_t cbit = s2 < s_star ? 1u : 0u;
+                        sumsq += cbit;
+                        w0 |= cbit << (8 * e);
+                    }
+                }
             }
-            pos += 32;
+            pos += 128;
         }
-        if (DIGITS == 1) {
-            sumsq += I;
-            base[kk * DG_SLAB] = (int8_t)I;
-            continue;
+        if (kk < ks) {
+            int8_t* p = base + kk * DIGITS * DG_SLAB;
+            *reinterpret_cast<uint32_t*>(p) = w0;
+            if (DIGITS == 3) {
+                *reinterpret_cast<uint32_t*>(p + DG_SLAB) = w1;
+                *reinterpret_cast<uint32_t*>(p + 2 * DG_SLAB) = w2;
+            }
         }
-        const int g2 = (int)(int8_t)(I & 0xff);
-        const int I1 = (I - g2) >> 8;
-        const int g1 = (int)(int8_t)(I1 & 0xff);
-        const int g0 = (I1 - g1) >> 8;
-        // |d|^2 from the SAME three levels the Gram keeps (I^2 minus the two dropped low-order levels), so that an
-        // identical pair cancels to exactly 0
-        sumsq += (long long)I * (long long)I - (long long)(512 * g1 * g2 + g2 * g2);
-        int8_t* p = base + kk * 3 * DG_SLAB;
-        p[0] = (int8_t)g0;
-        p[DG_SLAB] = (int8_t)g1;
-        p[2 * DG_SLAB] = (int8_t)g2;
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sumsq += __shfl_xor_sync(0xffffffffu, sumsq, o);
