@@ -36,6 +36,11 @@ _LIB_C = os.path.join(_HERE, "libcmo_oracle.so")
 _lib_c = None
 
 
+_SRC_G = os.path.join(_HERE, "gdt_oracle.c")
+_LIB_G = os.path.join(_HERE, "libgdt_oracle.so")
+_lib_g = None
+
+
 def _compile(src: str, lib: str, force: bool) -> str:
     if force or not os.path.exists(lib) or os.path.getmtime(lib) < os.path.getmtime(src):
         tmp = lib + f".tmp{os.getpid()}"
@@ -49,6 +54,7 @@ def build(force: bool = False) -> str:
     """Compile crmsd_oracle.c and drmsd_oracle.c (gcc -O2 -fopenmp, no fast-math); returns the cRMSD library."""
     _compile(_SRC_D, _LIB_D, force)
     _compile(_SRC_C, _LIB_C, force)
+    _compile(_SRC_G, _LIB_G, force)
     return _compile(_SRC, _LIB, force)
 
 
@@ -337,3 +343,35 @@ def cmo_pairs(coords, cutoff, pi, pj):
     s = np.empty(pi.size, np.float64)
     _load_c().oracle_cmo_pairs(_p(x, _f32p), N, L, _cut(cutoff), _p(pi, _i64p), _p(pj, _i64p), pi.size, _p(s, _f64p))
     return s
+
+
+# ---- GDT_TS / TM-score / MaxSub versus a reference (gdt_oracle.c) ------------------
+def _load_g():
+    global _lib_g
+    if _lib_g is None:
+        lib = ctypes.CDLL(_compile(_SRC_G, _LIB_G, False))
+        lib.oracle_gdt_pair.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p, _f64p]
+        lib.oracle_gdt_pair.restype = None
+        lib.oracle_gdt_one_vs_all.argtypes = [_f32p, _f32p, ctypes.c_int64, ctypes.c_int32, _f64p]
+        lib.oracle_gdt_one_vs_all.restype = None
+        _lib_g = lib
+    return _lib_g
+
+
+def gdt_pair(ref, model):
+    """The paper's search for one model: ((GDT_TS %, TM-score, MaxSub), max counts C_1, C_2, C_4, C_8)."""
+    a, b = _f32(ref), _f32(model)
+    assert a.shape == b.shape
+    out = np.empty(3, np.float64)
+    cnt = np.empty(4, np.float64)
+    _load_g().oracle_gdt_pair(_p(a, _f32p), _p(b, _f32p), a.shape[0], _p(out, _f64p), _p(cnt, _f64p))
+    return out, cnt
+
+
+def gdt_one_vs_all(ref, coords):
+    """Reference against coords[N][L][3]: float64 [N, 3] = (GDT_TS %, TM-score, MaxSub) per model."""
+    a, x = _f32(ref), _f32(coords)
+    N, L, _ = x.shape
+    out = np.empty((N, 3), np.float64)
+    _load_g().oracle_gdt_one_vs_all(_p(a, _f32p), _p(x, _f32p), N, L, _p(out, _f64p))
+    return out
