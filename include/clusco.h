@@ -171,6 +171,21 @@ int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N,
                             float* out, void* stream);
 
 /*
+ * GDT_TS, TM-score and MaxSub of N models against one reference structure (eq. 3-4), by the paper's
+ * search: every continuous fragment of length 4, L/4, L/2 and L seeds a superposition of the whole model (optimal
+ * rigid fit of the fragment); the atoms closer than 3.5 A are superposed again "until the number of selected atoms
+ * does not change in four iterations"; after every superposition
+ *     C_x = number of atom pairs below x = 1, 2, 4, 8 A,   TM = (1/L) sum_i 1 / (1 + (d_i/d0)^2),
+ *     d0 = 1.24 cbrt(L - 15) - 1.8 (clamped at 0.5 A);  MaxSub: the same with d0 = 3.5 A
+ * are evaluated and the maxima kept.  out[N][3] (float32): out[3n] = GDT_TS = 100 * (max C_1 + max C_2 + max C_4 +
+ * max C_8) / (4 L) in percent, out[3n+1] = TM-score, out[3n+2] = MaxSub.  native[L][3], coords[N][L][3], neither
+ * pre-superposed.  Readings of the points the paper leaves open (duplicate fragment lengths, iteration cap of 20,
+ * at least 3 selected atoms, strict inequalities): DESIGN.md section 14.  The search is data dependent, so the
+ * kernel works in FP64 throughout.  3 <= L <= 1024.  NaN/Inf coordinates give NaN for that model.
+ */
+int clusco_gdt_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream);
+
+/*
  * Host-buffer calls (blocking; the end-to-end path): coords_host / native_host / out_host are ordinary host
  * pointers -- pinned (page-locked) memory lets the transfers overlap the kernels, pageable memory works
  * but serialises.  Device scratch (inputs, result, workspace) is taken from a library-owned

@@ -27,6 +27,7 @@ EXPORTS = (
     "clusco_partition_rows", "clusco_engine_supported", "clusco_allpairs_prepare", "clusco_allpairs_compute",
     "clusco_host_release", "clusco_crmsd_allpairs_below", "clusco_crmsd_rowstats",
     "clusco_drmsd_allpairs_workspace", "clusco_drmsd_allpairs", "clusco_cmo_allpairs_workspace", "clusco_cmo_allpairs",
+    "clusco_gdt_one_vs_all",
 )
 
 
@@ -75,6 +76,7 @@ def load(build_if_missing: bool = False):
     lib.clusco_cmo_allpairs_workspace.argtypes = [i64, i32]
     lib.clusco_cmo_allpairs_workspace.restype = sz
     lib.clusco_cmo_allpairs.argtypes = [vp, i64, i32, ctypes.c_float, vp, vp, sz, vp]
+    lib.clusco_gdt_one_vs_all.argtypes = [vp, vp, i64, i32, vp, vp]
     for name in EXPORTS:                       # every declared symbol must be exported
         getattr(lib, name)
     _lib = lib
@@ -266,6 +268,21 @@ def clusco_crmsd_one_vs_all(native, coords, out=None):
     with torch.cuda.device(coords.device):
         st = load().clusco_crmsd_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_crmsd_one_vs_all")
+    return out
+
+
+def clusco_gdt_one_vs_all(native, coords, out=None):
+    """GDT_TS (percent), TM-score, MaxSub of coords[N][L][3] against native[L][3] -> float32 [N, 3] (include/clusco.h)."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    if not (native.is_cuda and native.dtype == torch.float32 and tuple(native.shape) == (L, 3)
+            and native.is_contiguous()):
+        raise CluscoError("native must be a contiguous CUDA float32 tensor of shape [L, 3]")
+    if out is None:
+        out = torch.empty((N, 3), dtype=torch.float32, device=coords.device)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_gdt_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
+    _check(st, "clusco_gdt_one_vs_all")
     return out
 
 

@@ -7,6 +7,7 @@
 
 #include "common.cuh"
 #include "epilogue.cuh"
+#include "gdt_ova.cuh"
 #include "gram_ffma.cuh"
 #include "drmsd_i8tc.cuh"
 #include "gram_i8tc.cuh"
@@ -318,6 +319,28 @@ int clusco_cmo_allpairs(const float* coords, int64_t N, int32_t L, float cutoff,
     const DWorkspace w = drmsd_workspace_layout(N, L, 1);
     if (!workspace || workspace_bytes < w.total || ((uintptr_t)workspace & 255u)) return CLUSCO_ERR_WORKSPACE_TOO_SMALL;
     return drmsd_launch<1>(coords, N, L, (double)cutoff, out, (char*)workspace, sms, s);
+}
+
+// NEXT-4: GDT_TS / TM-score / MaxSub of N models against one reference (the paper's fragment-seeded search, FP64)
+int clusco_gdt_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream)
+{
+    if (N < 0 || L < 3 || L > GDT_MAX_L) return CLUSCO_ERR_INVALID_ARG;
+    if (N == 0) return CLUSCO_OK;
+    if (!native || !coords || !out) return CLUSCO_ERR_INVALID_ARG;
+    int sms = 0;
+    int st = check_device(&sms);
+    if (st != CLUSCO_OK) return st;
+    const size_t smem = (size_t)(1 + GDT_WARPS) * 3 * (size_t)L * sizeof(double);
+    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gdt_one_vs_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 1;
+    CLUSCO_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gdt_one_vs_all_kernel, GDT_WARPS * 32, smem));
+    if (per_sm < 1) per_sm = 1;
+    int64_t grid = (N + GDT_WARPS - 1) / GDT_WARPS;
+    const int64_t cap = (int64_t)sms * per_sm;
+    if (grid > cap) grid = cap;
+    gdt_one_vs_all_kernel<<<(unsigned)grid, GDT_WARPS * 32, smem, (cudaStream_t)stream>>>(native, coords, N, L, out);
+    CLUSCO_CUDA_TRY(cudaGetLastError());
+    return CLUSCO_OK;
 }
 
 // one launch, no scratch: every CTA centres the native into its own shared memory
