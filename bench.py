@@ -279,11 +279,13 @@ def main():
     consumers = None
     drmsd = None
     cmo = None
+    gdt = None
     if not args.no_ova and world == 1:
         consumers = consumers_side(clusco, coords, ws, flush, P, ms_per_step)
         del ws
         drmsd = drmsd_side(clusco, coords, out, flush, N, L, P, pk)
         cmo = cmo_side(clusco, coords, out, flush, N, L, P, pk)
+        gdt = gdt_side(clusco, wl)
 
     cpu = None
     if not args.no_cpu_baseline:
@@ -299,7 +301,7 @@ def main():
                    "engine": {1: "ffma", 2: "i8tc"}[engine], "l2": "flushed between timed iterations (256 MB write)",
                    "effective_tflops": flops * world / (ms_per_step * 1e-3) / 1e12},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step(engine) * args.steps,
-        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova, "consumers": consumers, "drmsd": drmsd, "cmo": cmo,
+        "roofline": roof, "cpu_baseline": cpu, "one_vs_all": ova, "consumers": consumers, "drmsd": drmsd, "cmo": cmo, "gdt": gdt,
     }))
     if dist:
         dist.destroy_process_group()
@@ -435,6 +437,32 @@ def cmo_side(clusco, coords, out, flush, N, L, P, pk):
             "roofline": {"bound": "tensor", "achieved": ops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TOP/s",
                          "frac": ops / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel<1> (+ drmsd_prep_kernel<1>)",
                          "workspace_bytes": int(ws.numel())}}
+
+
+def gdt_side(clusco, wl):
+    """NEXT-4: GDT_TS / TM-score / MaxSub of the first 20 000 models of C5 (L=150) against the native --
+    the paper's fragment-seeded iterative search, FP64, one warp per model.  Data-dependent work: reported as models/s."""
+    import torch
+    N = 20_000
+    ens = wl.make_config("C5", N=N, chunk=N)
+    native = torch.from_numpy(ens.native).cuda()
+    coords = torch.from_numpy(ens.coords).cuda()
+    out = torch.empty((N, 3), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream()
+    clusco.clusco_gdt_one_vs_all(native, coords, out)
+    reps = 3
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    torch.cuda.synchronize()
+    for a, b in ev:
+        a.record(stream)
+        clusco.clusco_gdt_one_vs_all(native, coords, out)
+        b.record(stream)
+    torch.cuda.synchronize()
+    ms = sum(a.elapsed_time(b) for a, b in ev) / reps
+    o = out.cpu().numpy()
+    return {"workload": f"GDT_TS / TM-score / MaxSub, 1 native vs first {N} models of C5 (L=150)", "ms": ms,
+            "models_per_s": N / (ms * 1e-3), "mean_gdt_ts": float(o[:, 0].mean()), "mean_tm_score": float(o[:, 1].mean()),
+            "kernel": "gdt_one_vs_all_kernel", "bound": "alu (FP64, data-dependent iteration count)"}
 
 
 def launches_per_step(engine):

@@ -72,3 +72,11 @@ def test_gdt_closed_forms_and_edges(clusco):
     y[1, 3, 1] = np.nan
     got = clusco.clusco_gdt_one_vs_all(_dev(a), _dev(y)).cpu().numpy()
     assert np.all(np.isnan(got[1])) and np.all(np.isfinite(got[0]))
+
+
+def test_gdt_c5_sample(clusco):
+    """A 1500-model slice of C5 (the one-vs-all workload, L = 150) against the oracle, model by model."""
+    ens = wl.make_config("C5", N=1500, chunk=1500)
+    want = oracle.gdt_one_vs_all(ens.native, ens.coords)
+    got = clusco.clusco_gdt_one_vs_all(_dev(ens.native), _dev(ens.coords)).cpu().numpy()
+    _check(got, want, "C5[:1500]")
