@@ -93,7 +93,7 @@ constexpr int I8_ROW_MODELS = 32;      // models per row tile: 4 TMEM quadrants 
 constexpr int I8_COL_MODELS = 16;      // models per column tile: MMA N = 3 x 16 = 48 per level block
 constexpr int I8_A_SLAB = 128 * 32;    // bytes of one (k-step, digit) A slab: 128 rows x 32 atoms, int8
 constexpr int I8_B_SLAB = 144 * 32;    // bytes of one k-step B slab: 3 digits x 48 rows x 32 atoms
-constexpr int I8_MAX_KSTEPS = 8;       // L <= 256: the A tile (3 digits x ksteps x 4 KB) stays resident in shared memory
+constexpr int I8_MAX_KSTEPS = 8;       // L <= 256: a row tile's A operand (3 digits x ksteps x 8 columns) stays resident in TMEM
 
 // ---- workspace layout --------------------------------------------------------------------------
 // [ ModelStat[Np] | PairStat[Np] | FFMA plane | i8 A planes | i8 B planes ]      Np = N rounded up to 128

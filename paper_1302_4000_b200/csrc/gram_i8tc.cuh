@@ -22,7 +22,9 @@
 // Roles: warp 0 = bulk-copy producer (operand planes are stored in HBM as shared-memory images in the
 // canonical K-major core-matrix layout, so tiles arrive by plain 1-D cp.async.bulk), warp 1 = MMA issuer
 // (one thread) and TMEM owner, warps 2..17 = two epilogue teams of 8 warps (4 TMEM quadrants x 2 column
-// halves) that alternate over tiles; three TMEM accumulator buffers of 144 columns.
+// halves) that alternate over tiles on two TMEM accumulator buffers of 144 columns; a row tile's A operand is moved
+// once from a shared-memory staging area into TMEM (tcgen05.cp, columns 288...) and read from there by every MMA.
+// The epilogue's sink is a template parameter: packed store (a5), threshold compaction, or row statistics.
 #pragma once
 #include "common.cuh"
 #include "epilogue.cuh"
