@@ -251,6 +251,8 @@ def _load_d():
         lib.oracle_drmsd_pairs.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, _i64p, _i64p, ctypes.c_int64,
                                            _f64p, _f64p]
         lib.oracle_drmsd_pairs.restype = None
+        lib.oracle_drmsd_one_vs_all.argtypes = [_f32p, _f32p, ctypes.c_int64, ctypes.c_int32, _f64p, _f64p]
+        lib.oracle_drmsd_one_vs_all.restype = None
         _lib_d = lib
     return _lib_d
 
@@ -305,6 +307,8 @@ def _load_c():
         lib.oracle_cmo_pairs.argtypes = [_f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, _i64p, _i64p,
                                          ctypes.c_int64, _f64p]
         lib.oracle_cmo_pairs.restype = None
+        lib.oracle_cmo_one_vs_all.argtypes = [_f32p, _f32p, ctypes.c_int64, ctypes.c_int32, ctypes.c_double, _f64p]
+        lib.oracle_cmo_one_vs_all.restype = None
         _lib_c = lib
     return _lib_c
 
@@ -375,3 +379,22 @@ def gdt_one_vs_all(ref, coords):
     out = np.empty((N, 3), np.float64)
     _load_g().oracle_gdt_one_vs_all(_p(a, _f32p), _p(x, _f32p), N, L, _p(out, _f64p))
     return out
+
+
+def drmsd_one_vs_all(ref, coords):
+    """eq. 5 of one reference against coords[N][L][3]: (d, d2) fp64 [N]."""
+    a, x = _f32(ref), _f32(coords)
+    N, L, _ = x.shape
+    d = np.empty(N, np.float64)
+    d2 = np.empty(N, np.float64)
+    _load_d().oracle_drmsd_one_vs_all(_p(a, _f32p), _p(x, _f32p), N, L, _p(d, _f64p), _p(d2, _f64p))
+    return d, d2
+
+
+def cmo_one_vs_all(ref, coords, cutoff):
+    """eq. 6-7 of one reference against coords[N][L][3]: S fp64 [N]."""
+    a, x = _f32(ref), _f32(coords)
+    N, L, _ = x.shape
+    s = np.empty(N, np.float64)
+    _load_c().oracle_cmo_one_vs_all(_p(a, _f32p), _p(x, _f32p), N, L, _cut(cutoff), _p(s, _f64p))
+    return s

@@ -60,3 +60,10 @@ void oracle_cmo_pairs(const float *coords, int64_t N, int32_t L, double cutoff, 
     for (int64_t k = 0; k < n_pairs; ++k)
         s_out[k] = oracle_cmo_pair(coords + (size_t)pi[k] * L * 3, coords + (size_t)pj[k] * L * 3, L, cutoff, 0);
 }
+
+/* One reference against N models: eq. 6-7 for (ref, model n). */
+void oracle_cmo_one_vs_all(const float *ref, const float *coords, int64_t N, int32_t L, double cutoff, double *s_out)
+{
+    #pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < N; ++n) s_out[n] = oracle_cmo_pair(ref, coords + (size_t)n * L * 3, L, cutoff, 0);
+}

@@ -72,3 +72,14 @@ void oracle_drmsd_pairs(const float *coords, int64_t N, int32_t L, const int64_t
         if (d2_out) d2_out[k] = d2;
     }
 }
+
+/* One reference against N models: eq. 5 for (ref, model n). */
+void oracle_drmsd_one_vs_all(const float *ref, const float *coords, int64_t N, int32_t L, double *d_out, double *d2_out)
+{
+    #pragma omp parallel for schedule(static)
+    for (int64_t n = 0; n < N; ++n) {
+        double d2;
+        d_out[n] = oracle_drmsd_pair(ref, coords + (size_t)n * L * 3, L, &d2);
+        if (d2_out) d2_out[n] = d2;
+    }
+}

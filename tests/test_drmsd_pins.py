@@ -103,3 +103,18 @@ def test_mirror_decoys_of_C1_are_close_in_drmsd_only():
     d = oracle.drmsd_pair(ens.coords[mi], ens.coords[other])[0]
     c = oracle.crmsd_pair(ens.coords[mi], ens.coords[other])[0]
     assert d < c and c > 10.0
+
+
+def test_one_vs_all_forms_match_pair_route():
+    ens = wl.make_config("C5", N=50, chunk=50)
+    d, d2 = oracle.drmsd_one_vs_all(ens.native, ens.coords)
+    s = oracle.cmo_one_vs_all(ens.native, ens.coords, 8.0)
+    for n in (0, 7, 49):
+        assert (d[n], d2[n]) == oracle.drmsd_pair(ens.native, ens.coords[n])
+        assert s[n] == oracle.cmo_pair(ens.native, ens.coords[n], 8.0)[0]
+    # closed form: the reference against itself and against its mirror image
+    m = ens.native.copy()
+    m[:, 2] = -m[:, 2]
+    d, _ = oracle.drmsd_one_vs_all(ens.native, np.stack([ens.native, m]))
+    assert d[0] == 0.0 and d[1] == 0.0
+    assert list(oracle.cmo_one_vs_all(ens.native, np.stack([ens.native, m]), 8.0)) == [100.0, 100.0]
