@@ -171,6 +171,16 @@ int clusco_crmsd_one_vs_all(const float* native, const float* coords, int64_t N,
                             float* out, void* stream);
 
 /*
+ * dRMSD (eq. 5) and contact map overlap (eq. 6-7) of N models against ONE reference structure ("... or with respect to
+ * the reference model"): out[n] = the measure of (native, model n), defined as in the
+ * all-versus-all calls above (same readings, same contact decision; CMO is bit-exact).  Single pass, FP64, one warp
+ * per model; 1 <= L <= 1024 (L = 1: dRMSD 0, CMO 100); cutoff >= 0.  NaN/Inf coordinates -> NaN for that model.
+ */
+int clusco_drmsd_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream);
+int clusco_cmo_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float cutoff, float* out,
+                          void* stream);
+
+/*
  * GDT_TS, TM-score and MaxSub of N models against one reference structure (eq. 3-4), by the paper's
  * search: every continuous fragment of length 4, L/4, L/2 and L seeds a superposition of the whole model (optimal
  * rigid fit of the fragment); the atoms closer than 3.5 A are superposed again "until the number of selected atoms

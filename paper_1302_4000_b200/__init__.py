@@ -27,7 +27,7 @@ EXPORTS = (
     "clusco_partition_rows", "clusco_engine_supported", "clusco_allpairs_prepare", "clusco_allpairs_compute",
     "clusco_host_release", "clusco_crmsd_allpairs_below", "clusco_crmsd_rowstats",
     "clusco_drmsd_allpairs_workspace", "clusco_drmsd_allpairs", "clusco_cmo_allpairs_workspace", "clusco_cmo_allpairs",
-    "clusco_gdt_one_vs_all",
+    "clusco_gdt_one_vs_all", "clusco_drmsd_one_vs_all", "clusco_cmo_one_vs_all",
 )
 
 
@@ -77,6 +77,8 @@ def load(build_if_missing: bool = False):
     lib.clusco_cmo_allpairs_workspace.restype = sz
     lib.clusco_cmo_allpairs.argtypes = [vp, i64, i32, ctypes.c_float, vp, vp, sz, vp]
     lib.clusco_gdt_one_vs_all.argtypes = [vp, vp, i64, i32, vp, vp]
+    lib.clusco_drmsd_one_vs_all.argtypes = [vp, vp, i64, i32, vp, vp]
+    lib.clusco_cmo_one_vs_all.argtypes = [vp, vp, i64, i32, ctypes.c_float, vp, vp]
     for name in EXPORTS:                       # every declared symbol must be exported
         getattr(lib, name)
     _lib = lib
@@ -268,6 +270,39 @@ def clusco_crmsd_one_vs_all(native, coords, out=None):
     with torch.cuda.device(coords.device):
         st = load().clusco_crmsd_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_crmsd_one_vs_all")
+    return out
+
+
+def _check_native(native, coords):
+    torch = _torch()
+    N, L = _check_coords(coords)
+    if not (native.is_cuda and native.dtype == torch.float32 and tuple(native.shape) == (L, 3)
+            and native.is_contiguous()):
+        raise CluscoError("native must be a contiguous CUDA float32 tensor of shape [L, 3]")
+    return N, L
+
+
+def clusco_drmsd_one_vs_all(native, coords, out=None):
+    """dRMSD (eq. 5) of coords[N][L][3] against native[L][3] -> float32[N]."""
+    torch = _torch()
+    N, L = _check_native(native, coords)
+    if out is None:
+        out = torch.empty(N, dtype=torch.float32, device=coords.device)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_drmsd_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
+    _check(st, "clusco_drmsd_one_vs_all")
+    return out
+
+
+def clusco_cmo_one_vs_all(native, coords, cutoff: float, out=None):
+    """Contact map overlap (eq. 6-7) of coords[N][L][3] against native[L][3] -> float32[N]."""
+    torch = _torch()
+    N, L = _check_native(native, coords)
+    if out is None:
+        out = torch.empty(N, dtype=torch.float32, device=coords.device)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_cmo_one_vs_all(_ptr(native), _ptr(coords), N, L, float(cutoff), _ptr(out), _stream_ptr(coords))
+    _check(st, "clusco_cmo_one_vs_all")
     return out
 
 

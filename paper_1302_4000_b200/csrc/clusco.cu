@@ -13,6 +13,7 @@
 #include "gram_i8tc.cuh"
 #include "one_vs_all.cuh"
 #include "prep.cuh"
+#include "ref_ova.cuh"
 
 namespace clusco {
 thread_local int g_last_cuda_error = 0;
@@ -319,6 +320,32 @@ int clusco_cmo_allpairs(const float* coords, int64_t N, int32_t L, float cutoff,
     const DWorkspace w = drmsd_workspace_layout(N, L, 1);
     if (!workspace || workspace_bytes < w.total || ((uintptr_t)workspace & 255u)) return CLUSCO_ERR_WORKSPACE_TOO_SMALL;
     return drmsd_launch<1>(coords, N, L, (double)cutoff, out, (char*)workspace, sms, s);
+}
+
+// dRMSD and CMO of N models against one reference (the versus-reference form of eq. 5 and eq. 6-7)
+static int ref_ova_common(int mode, const float* native, const float* coords, int64_t N, int32_t L, double cutoff, float* out,
+                          void* stream)
+{
+    if (N < 0 || L < 1 || L > ROVA_MAX_L) return CLUSCO_ERR_INVALID_ARG;
+    if (N == 0) return CLUSCO_OK;
+    if (!native || !coords || !out) return CLUSCO_ERR_INVALID_ARG;
+    int sms = 0;
+    int st = check_device(&sms);
+    if (st != CLUSCO_OK) return st;
+    return mode == 0 ? ref_one_vs_all_launch<0>(native, coords, N, L, cutoff, out, sms, (cudaStream_t)stream)
+                     : ref_one_vs_all_launch<1>(native, coords, N, L, cutoff, out, sms, (cudaStream_t)stream);
+}
+
+int clusco_drmsd_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream)
+{
+    return ref_ova_common(0, native, coords, N, L, 0.0, out, stream);
+}
+
+int clusco_cmo_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float cutoff, float* out,
+                          void* stream)
+{
+    if (!(cutoff >= 0.0f)) return CLUSCO_ERR_INVALID_ARG;
+    return ref_ova_common(1, native, coords, N, L, (double)cutoff, out, stream);
 }
 
 // NEXT-4: GDT_TS / TM-score / MaxSub of N models against one reference (the paper's fragment-seeded search, FP64)

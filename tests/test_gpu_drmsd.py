@@ -110,3 +110,30 @@ def test_drmsd_cluster_path_every_pair(clusco, N, L):
     d_ref, d2_ref = oracle.drmsd_allpairs(x)
     got = clusco.clusco_drmsd_allpairs(_dev(x)).cpu().numpy()
     _check(got, d_ref, d2_ref, f"cluster N={N} L={L}")
+
+
+@pytest.mark.parametrize("N,L", [(2000, 150), (65, 33), (7, 2), (40, 300)])
+def test_drmsd_and_cmo_one_vs_all(clusco, N, L):
+    """The versus-reference forms: dRMSD within the pair tolerance, CMO bit-exact."""
+    if L == 150:
+        ens = wl.make_config("C5", N=N, chunk=N)
+        native, x = ens.native, ens.coords
+    else:
+        rng = np.random.default_rng(L)
+        native = wl.random_walk_chain(L, rng)
+        x = np.stack([wl.rigid_transform((native + rng.normal(size=native.shape) * rng.uniform(0.3, 6.0))[None], rng)[0]
+                      for _ in range(N)]).astype(np.float32)
+        native = native.astype(np.float32)
+    d_ref, d2_ref = oracle.drmsd_one_vs_all(native, x)
+    got = clusco.clusco_drmsd_one_vs_all(_dev(native), _dev(x)).cpu().numpy()
+    _check(got, d_ref, d2_ref, f"dRMSD one-vs-all N={N} L={L}")
+    s_ref = oracle.cmo_one_vs_all(native, x, 8.0).astype(np.float32)
+    s = clusco.clusco_cmo_one_vs_all(_dev(native), _dev(x), 8.0).cpu().numpy()
+    assert np.array_equal(s, s_ref)
+    # against itself / NaN model
+    self_d = clusco.clusco_drmsd_one_vs_all(_dev(native), _dev(native[None])).cpu().numpy()
+    assert self_d[0] == 0.0
+    y = x[:3].copy()
+    y[1, 0, 0] = np.nan
+    assert np.isnan(clusco.clusco_drmsd_one_vs_all(_dev(native), _dev(y)).cpu().numpy()[1])
+    assert np.isnan(clusco.clusco_cmo_one_vs_all(_dev(native), _dev(y), 8.0).cpu().numpy()[1])
