@@ -467,7 +467,7 @@ def gdt_side(clusco, wl):
     o = out.cpu().numpy()
     return {"workload": f"GDT_TS / TM-score / MaxSub, 1 native vs first {N} models of C5 (L=150)", "ms": ms,
             "models_per_s": N / (ms * 1e-3), "mean_gdt_ts": float(o[:, 0].mean()), "mean_tm_score": float(o[:, 1].mean()),
-            "kernel": "gdt_one_vs_all_kernel", "bound": "alu (FP64, data-dependent iteration count)"}
+            "kernel": "gdt_kernel<false>", "bound": "alu (FP64, data-dependent iteration count)"}
 
 
 def launches_per_step(engine):

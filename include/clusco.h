@@ -194,6 +194,13 @@ int clusco_cmo_one_vs_all(const float* native, const float* coords, int64_t N, i
  * kernel works in FP64 throughout.  3 <= L <= 1024.  NaN/Inf coordinates give NaN for that model.
  */
 int clusco_gdt_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream);
+/*
+ * The same three scores all-versus-all: out[N(N-1)/2][3], packed row-major upper triangle as in
+ * clusco_crmsd_allpairs; for the pair i < j model i plays the reference (the search is symmetric in the two
+ * structures -- selections depend on distances only -- so the scores are those of (j, i) too).  One warp per pair;
+ * the cost is ~5 us of FP64 work per pair at L = 150, so this is meant for thousands of models, not millions.
+ */
+int clusco_gdt_allpairs(const float* coords, int64_t N, int32_t L, float* out, void* stream);
 
 /*
  * Host-buffer calls (blocking; the end-to-end path): coords_host / native_host / out_host are ordinary host

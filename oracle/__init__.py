@@ -398,3 +398,11 @@ def cmo_one_vs_all(ref, coords, cutoff):
     s = np.empty(N, np.float64)
     _load_c().oracle_cmo_one_vs_all(_p(a, _f32p), _p(x, _f32p), N, L, _cut(cutoff), _p(s, _f64p))
     return s
+
+
+def gdt_allpairs(coords):
+    """All-versus-all form: for i < j model i is the reference; float64 [N(N-1)/2, 3], packed row-major."""
+    x = _f32(coords)
+    N = x.shape[0]
+    rows = [gdt_one_vs_all(x[i], x[i + 1:]) for i in range(N - 1)]
+    return np.concatenate(rows) if rows else np.zeros((0, 3))

@@ -27,7 +27,7 @@ EXPORTS = (
     "clusco_partition_rows", "clusco_engine_supported", "clusco_allpairs_prepare", "clusco_allpairs_compute",
     "clusco_host_release", "clusco_crmsd_allpairs_below", "clusco_crmsd_rowstats",
     "clusco_drmsd_allpairs_workspace", "clusco_drmsd_allpairs", "clusco_cmo_allpairs_workspace", "clusco_cmo_allpairs",
-    "clusco_gdt_one_vs_all", "clusco_drmsd_one_vs_all", "clusco_cmo_one_vs_all",
+    "clusco_gdt_one_vs_all", "clusco_drmsd_one_vs_all", "clusco_cmo_one_vs_all", "clusco_gdt_allpairs",
 )
 
 
@@ -79,6 +79,7 @@ def load(build_if_missing: bool = False):
     lib.clusco_gdt_one_vs_all.argtypes = [vp, vp, i64, i32, vp, vp]
     lib.clusco_drmsd_one_vs_all.argtypes = [vp, vp, i64, i32, vp, vp]
     lib.clusco_cmo_one_vs_all.argtypes = [vp, vp, i64, i32, ctypes.c_float, vp, vp]
+    lib.clusco_gdt_allpairs.argtypes = [vp, i64, i32, vp, vp]
     for name in EXPORTS:                       # every declared symbol must be exported
         getattr(lib, name)
     _lib = lib
@@ -318,6 +319,18 @@ def clusco_gdt_one_vs_all(native, coords, out=None):
     with torch.cuda.device(coords.device):
         st = load().clusco_gdt_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_gdt_one_vs_all")
+    return out
+
+
+def clusco_gdt_allpairs(coords, out=None):
+    """All-versus-all GDT_TS (percent), TM-score, MaxSub -> float32 [N(N-1)/2, 3], packed upper triangle."""
+    torch = _torch()
+    N, L = _check_coords(coords)
+    if out is None:
+        out = torch.empty((n_pairs(N), 3), dtype=torch.float32, device=coords.device)
+    with torch.cuda.device(coords.device):
+        st = load().clusco_gdt_allpairs(_ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
+    _check(st, "clusco_gdt_allpairs")
     return out
 
 

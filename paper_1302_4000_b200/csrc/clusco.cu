@@ -348,26 +348,45 @@ int clusco_cmo_one_vs_all(const float* native, const float* coords, int64_t N, i
     return ref_ova_common(1, native, coords, N, L, (double)cutoff, out, stream);
 }
 
-// NEXT-4: GDT_TS / TM-score / MaxSub of N models against one reference (the paper's fragment-seeded search, FP64)
+// NEXT-4: GDT_TS / TM-score / MaxSub (the paper's fragment-seeded search, FP64): versus a reference, and all-versus-all
+}  // extern "C"
+
+template <bool ALLPAIRS>
+static int gdt_launch(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream)
+{
+    int sms = 0;
+    int st = check_device(&sms);
+    if (st != CLUSCO_OK) return st;
+    const size_t smem = (size_t)(ALLPAIRS ? 2 * GDT_WARPS : 1 + GDT_WARPS) * 3 * (size_t)L * sizeof(double);
+    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gdt_kernel<ALLPAIRS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 1;
+    CLUSCO_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gdt_kernel<ALLPAIRS>, GDT_WARPS * 32, smem));
+    if (per_sm < 1) per_sm = 1;
+    const int64_t units = ALLPAIRS ? N * (N - 1) / 2 : N;
+    int64_t grid = (units + GDT_WARPS - 1) / GDT_WARPS;
+    const int64_t cap = (int64_t)sms * per_sm;
+    if (grid > cap) grid = cap;
+    gdt_kernel<ALLPAIRS><<<(unsigned)grid, GDT_WARPS * 32, smem, (cudaStream_t)stream>>>(native, coords, N, L, out);
+    CLUSCO_CUDA_TRY(cudaGetLastError());
+    return CLUSCO_OK;
+}
+
+extern "C" {
+
 int clusco_gdt_one_vs_all(const float* native, const float* coords, int64_t N, int32_t L, float* out, void* stream)
 {
     if (N < 0 || L < 3 || L > GDT_MAX_L) return CLUSCO_ERR_INVALID_ARG;
     if (N == 0) return CLUSCO_OK;
     if (!native || !coords || !out) return CLUSCO_ERR_INVALID_ARG;
-    int sms = 0;
-    int st = check_device(&sms);
-    if (st != CLUSCO_OK) return st;
-    const size_t smem = (size_t)(1 + GDT_WARPS) * 3 * (size_t)L * sizeof(double);
-    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(gdt_one_vs_all_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int per_sm = 1;
-    CLUSCO_CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gdt_one_vs_all_kernel, GDT_WARPS * 32, smem));
-    if (per_sm < 1) per_sm = 1;
-    int64_t grid = (N + GDT_WARPS - 1) / GDT_WARPS;
-    const int64_t cap = (int64_t)sms * per_sm;
-    if (grid > cap) grid = cap;
-    gdt_one_vs_all_kernel<<<(unsigned)grid, GDT_WARPS * 32, smem, (cudaStream_t)stream>>>(native, coords, N, L, out);
-    CLUSCO_CUDA_TRY(cudaGetLastError());
-    return CLUSCO_OK;
+    return gdt_launch<false>(native, coords, N, L, out, stream);
+}
+
+int clusco_gdt_allpairs(const float* coords, int64_t N, int32_t L, float* out, void* stream)
+{
+    if (N < 0 || L < 3 || L > GDT_MAX_L || N > (int64_t)1 << 24) return CLUSCO_ERR_INVALID_ARG;
+    if (N < 2) return CLUSCO_OK;
+    if (!coords || !out) return CLUSCO_ERR_INVALID_ARG;
+    return gdt_launch<true>(nullptr, coords, N, L, out, stream);
 }
 
 // one launch, no scratch: every CTA centres the native into its own shared memory

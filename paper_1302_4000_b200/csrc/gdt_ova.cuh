@@ -115,16 +115,35 @@ __device__ __forceinline__ double gdt_warp_sum(double v)
 // out[3 n + {0, 1, 2}] = GDT_TS (percent), TM-score, MaxSub of model n against the reference.
 // Dynamic shared memory: (1 + GDT_WARPS) * 3 L doubles -- the reference and one model per warp, each centred on its own
 // centroid (rigid motions do not change the scores; centring keeps the covariance sums free of cancellation).
-__global__ void __launch_bounds__(GDT_WARPS * 32) gdt_one_vs_all_kernel(const float* __restrict__ ref,
-                                                                        const float* __restrict__ coords, int64_t N, int32_t L,
-                                                                        float* __restrict__ out)
+// ALLPAIRS: unit = pair (i < j) of the packed upper triangle, reference = model i (the search is symmetric in the two
+// structures: selections depend on distances only), out[3 idx + ...] with idx the packed index; both models per warp.
+template <bool ALLPAIRS>
+__global__ void __launch_bounds__(GDT_WARPS * 32) gdt_kernel(const float* __restrict__ ref, const float* __restrict__ coords,
+                                                             int64_t N, int32_t L, float* __restrict__ out)
 {
     extern __shared__ __align__(16) double gdt_smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double* A = gdt_smem;                                        // reference, 3 L
-    double* B = gdt_smem + (size_t)(1 + warp) * 3 * L;           // this warp's model
-    // reference: every CTA centres it itself (FP64)
-    {
+    double* A = ALLPAIRS ? gdt_smem + (size_t)(2 * warp) * 3 * L : gdt_smem;                       // reference, 3 L
+    double* B = ALLPAIRS ? gdt_smem + (size_t)(2 * warp + 1) * 3 * L : gdt_smem + (size_t)(1 + warp) * 3 * L;
+    // centre a model (FP64) into shared memory; returns whether all its coordinates are finite
+    auto load_centred = [&](double* dst, const float* x) {
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+        bool fin = true;
+        for (int i = lane; i < L; i += 32) {
+            const float v0 = x[3 * i], v1 = x[3 * i + 1], v2 = x[3 * i + 2];
+            fin = fin && fabsf(v0) <= 3.0e38f && fabsf(v1) <= 3.0e38f && fabsf(v2) <= 3.0e38f;
+            s0 += (double)v0; s1 += (double)v1; s2 += (double)v2;
+        }
+        s0 = gdt_warp_sum(s0) / (double)L; s1 = gdt_warp_sum(s1) / (double)L; s2 = gdt_warp_sum(s2) / (double)L;
+        __syncwarp();
+        for (int i = lane; i < L; i += 32) {
+            dst[3 * i] = (double)x[3 * i] - s0; dst[3 * i + 1] = (double)x[3 * i + 1] - s1; dst[3 * i + 2] = (double)x[3 * i + 2] - s2;
+        }
+        __syncwarp();
+        return (bool)__all_sync(0xffffffffu, fin);
+    };
+    // one-vs-all: every CTA centres the reference itself (FP64)
+    if (!ALLPAIRS) {
         __shared__ double red[3][GDT_WARPS];
         double s0 = 0.0, s1 = 0.0, s2 = 0.0;
         for (int i = threadIdx.x; i < L; i += blockDim.x) { s0 += (double)ref[3 * i]; s1 += (double)ref[3 * i + 1]; s2 += (double)ref[3 * i + 2]; }
@@ -143,23 +162,21 @@ __global__ void __launch_bounds__(GDT_WARPS * 32) gdt_one_vs_all_kernel(const fl
     int lens[4] = {4, L / 4, L / 2, L};
     if (L < 4) lens[0] = lens[1] = lens[2] = L;
 
-    for (int64_t n = (int64_t)blockIdx.x * GDT_WARPS + warp; n < N; n += (int64_t)gridDim.x * GDT_WARPS) {
-        // load + centre the model
-        const float* x = coords + n * (int64_t)L * 3;
-        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    const int64_t total = ALLPAIRS ? N * (N - 1) / 2 : N;
+    for (int64_t n = (int64_t)blockIdx.x * GDT_WARPS + warp; n < total; n += (int64_t)gridDim.x * GDT_WARPS) {
         bool finite = true;
-        for (int i = lane; i < L; i += 32) {
-            const float v0 = x[3 * i], v1 = x[3 * i + 1], v2 = x[3 * i + 2];
-            finite = finite && fabsf(v0) <= 3.0e38f && fabsf(v1) <= 3.0e38f && fabsf(v2) <= 3.0e38f;
-            s0 += (double)v0; s1 += (double)v1; s2 += (double)v2;
+        int64_t jm = n;                                          // the model superposed onto the reference
+        if (ALLPAIRS) {
+            // packed index n -> (i, j): row i starts at i (2N - i - 1) / 2
+            const double Nd = (double)N;
+            int64_t i = (int64_t)floor(((2.0 * Nd - 1.0) - sqrt((2.0 * Nd - 1.0) * (2.0 * Nd - 1.0) - 8.0 * (double)n)) * 0.5);
+            if (i < 0) i = 0;
+            while (i > 0 && i * (2 * N - i - 1) / 2 > n) --i;
+            while ((i + 1) * (2 * N - i - 2) / 2 <= n) ++i;
+            jm = i + 1 + (n - i * (2 * N - i - 1) / 2);
+            finite = load_centred(A, coords + i * (int64_t)L * 3);
         }
-        s0 = gdt_warp_sum(s0) / (double)L; s1 = gdt_warp_sum(s1) / (double)L; s2 = gdt_warp_sum(s2) / (double)L;
-        finite = __all_sync(0xffffffffu, finite);
-        __syncwarp();
-        for (int i = lane; i < L; i += 32) {
-            B[3 * i] = (double)x[3 * i] - s0; B[3 * i + 1] = (double)x[3 * i + 1] - s1; B[3 * i + 2] = (double)x[3 * i + 2] - s2;
-        }
-        __syncwarp();
+        finite = load_centred(B, coords + jm * (int64_t)L * 3) && finite;
         int bestc0 = 0, bestc1 = 0, bestc2 = 0, bestc3 = 0;
         double best_tm = 0.0, best_ms = 0.0;
         for (int f = 0; f < 4; ++f) {

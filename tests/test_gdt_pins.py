@@ -83,3 +83,23 @@ def test_lower_bound_from_library_kabsch_and_invariance():
         assert abs(s2[1] - s[1]) < 1e-4 and abs(s2[0] - s[0]) <= 100.0 / L + 1e-9
     out = oracle.gdt_one_vs_all(a32, np.stack([b32, a32]))
     assert np.allclose(out[0], s) and out[1][0] == 100.0
+
+
+def test_allpairs_form_is_symmetric_in_the_two_structures():
+    """PAPER.md:84 (all-versus-all): the packed form takes model i as the reference of pair i < j.  The search selects
+    atoms by distances only, so exchanging the two structures gives the same counts and scores (up to rounding of the
+    inverse rotation): check the packed result against the pair routine called BOTH ways, and its shape and order."""
+    rng = np.random.default_rng(11)
+    a = _chain(40, 5)
+    x = np.stack([_rigid(a + rng.normal(size=a.shape) * s, rng) for s in (0.0, 0.6, 1.5, 3.0, 6.0)]).astype(np.float32)
+    out = oracle.gdt_allpairs(x)
+    assert out.shape == (10, 3)
+    k = 0
+    for i in range(5):
+        for j in range(i + 1, 5):
+            sij, cij = oracle.gdt_pair(x[i], x[j])
+            sji, cji = oracle.gdt_pair(x[j], x[i])
+            assert np.allclose(out[k], sij, atol=1e-12)
+            assert abs(sij[0] - sji[0]) <= 100.0 / 40 / 4 + 1e-9 and np.allclose(sij[1:], sji[1:], atol=1e-6)
+            k += 1
+    assert oracle.gdt_allpairs(x[:1]).shape == (0, 3)

@@ -80,3 +80,13 @@ def test_gdt_c5_sample(clusco):
     want = oracle.gdt_one_vs_all(ens.native, ens.coords)
     got = clusco.clusco_gdt_one_vs_all(_dev(ens.native), _dev(ens.coords)).cpu().numpy()
     _check(got, want, "C5[:1500]")
+
+
+@pytest.mark.parametrize("cfg,N", [("C1", 60), ("C2", 40)])
+def test_gdt_allpairs(clusco, cfg, N):
+    """All-versus-all form: every pair against the oracle run pair by pair (model i as the reference)."""
+    ens = wl.make_config(cfg, N=N)
+    want = oracle.gdt_allpairs(ens.coords)
+    got = clusco.clusco_gdt_allpairs(_dev(ens.coords)).cpu().numpy()
+    _check(got, want, f"{cfg} all pairs")
+    assert clusco.clusco_gdt_allpairs(_dev(ens.coords[:1])).shape == (0, 3)
