@@ -112,6 +112,26 @@ __device__ __forceinline__ double gdt_warp_sum(double v)
     return v;
 }
 
+// centre a model (FP64) into shared memory, one warp; returns whether all its coordinates are finite
+__device__ __forceinline__ bool gdt_load_centred(double* __restrict__ dst, const float* __restrict__ x, int L, int lane)
+{
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    bool fin = true;
+    for (int i = lane; i < L; i += 32) {
+        const float v0 = x[3 * i], v1 = x[3 * i + 1], v2 = x[3 * i + 2];
+        fin = fin && fabsf(v0) <= 3.0e38f && fabsf(v1) <= 3.0e38f && fabsf(v2) <= 3.0e38f;
+        s0 += (double)v0; s1 += (double)v1; s2 += (double)v2;
+    }
+    s0 = gdt_warp_sum(s0) / (double)L; s1 = gdt_warp_sum(s1) / (double)L; s2 = gdt_warp_sum(s2) / (double)L;
+    fin = __all_sync(0xffffffffu, fin);
+    __syncwarp();
+    for (int i = lane; i < L; i += 32) {
+        dst[3 * i] = (double)x[3 * i] - s0; dst[3 * i + 1] = (double)x[3 * i + 1] - s1; dst[3 * i + 2] = (double)x[3 * i + 2] - s2;
+    }
+    __syncwarp();
+    return fin;
+}
+
 // out[3 n + {0, 1, 2}] = GDT_TS (percent), TM-score, MaxSub of model n against the reference.
 // Dynamic shared memory: (1 + GDT_WARPS) * 3 L doubles -- the reference and one model per warp, each centred on its own
 // centroid (rigid motions do not change the scores; centring keeps the covariance sums free of cancellation).
@@ -125,23 +145,6 @@ __global__ void __launch_bounds__(GDT_WARPS * 32) gdt_kernel(const float* __rest
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     double* A = ALLPAIRS ? gdt_smem + (size_t)(2 * warp) * 3 * L : gdt_smem;                       // reference, 3 L
     double* B = ALLPAIRS ? gdt_smem + (size_t)(2 * warp + 1) * 3 * L : gdt_smem + (size_t)(1 + warp) * 3 * L;
-    // centre a model (FP64) into shared memory; returns whether all its coordinates are finite
-    auto load_centred = [&](double* dst, const float* x) {
-        double s0 = 0.0, s1 = 0.0, s2 = 0.0;
-        bool fin = true;
-        for (int i = lane; i < L; i += 32) {
-            const float v0 = x[3 * i], v1 = x[3 * i + 1], v2 = x[3 * i + 2];
-            fin = fin && fabsf(v0) <= 3.0e38f && fabsf(v1) <= 3.0e38f && fabsf(v2) <= 3.0e38f;
-            s0 += (double)v0; s1 += (double)v1; s2 += (double)v2;
-        }
-        s0 = gdt_warp_sum(s0) / (double)L; s1 = gdt_warp_sum(s1) / (double)L; s2 = gdt_warp_sum(s2) / (double)L;
-        __syncwarp();
-        for (int i = lane; i < L; i += 32) {
-            dst[3 * i] = (double)x[3 * i] - s0; dst[3 * i + 1] = (double)x[3 * i + 1] - s1; dst[3 * i + 2] = (double)x[3 * i + 2] - s2;
-        }
-        __syncwarp();
-        return (bool)__all_sync(0xffffffffu, fin);
-    };
     // one-vs-all: every CTA centres the reference itself (FP64)
     if (!ALLPAIRS) {
         __shared__ double red[3][GDT_WARPS];
@@ -174,9 +177,9 @@ __global__ void __launch_bounds__(GDT_WARPS * 32) gdt_kernel(const float* __rest
             while (i > 0 && i * (2 * N - i - 1) / 2 > n) --i;
             while ((i + 1) * (2 * N - i - 2) / 2 <= n) ++i;
             jm = i + 1 + (n - i * (2 * N - i - 1) / 2);
-            finite = load_centred(A, coords + i * (int64_t)L * 3);
+            finite = gdt_load_centred(A, coords + i * (int64_t)L * 3, L, lane);
         }
-        finite = load_centred(B, coords + jm * (int64_t)L * 3) && finite;
+        finite = gdt_load_centred(B, coords + jm * (int64_t)L * 3, L, lane) && finite;
         int bestc0 = 0, bestc1 = 0, bestc2 = 0, bestc3 = 0;
         double best_tm = 0.0, best_ms = 0.0;
         for (int f = 0; f < 4; ++f) {
