@@ -19,8 +19,8 @@
 //
 // Kernel: persistent, one CTA per SM, tile = 128 x 128 models, warp 0 = bulk-copy producer (ring of stages of KG
 // k-steps: A and B, each KG x DIGITS x 4 KB), warp 1 = MMA issuer -- per k-step six N = 128 MMAs, level v (TMEM columns
-// 128 v ...) collecting the digit products A(ga).B(gb)^T with ga + gb = v -- warps 2..5 = epilogue (FP64: the K loop
-// is ~1000 k-steps long, the epilogue is <1 % of a tile).  2 x 2 thread-block clusters multicast the operands (below).
+// 128 v ...) collecting the digit products A(ga).B(gb)^T with ga + gb = v -- warps 2..17 = epilogue (quadrant x
+// column quarter; results are transposed through shared memory so that the stores run along the packed rows).  2 x 2 thread-block clusters multicast the operands (below).
 #pragma once
 #include "common.cuh"
 #include "prep.cuh"
@@ -42,7 +42,17 @@ template <int DIGITS> struct DGCfg {
     static constexpr int STAGE_BYTES = 2 * OPER_BYTES;
     static constexpr int STAGES = (216 * 1024) / STAGE_BYTES;
 };
-constexpr int DG_THREADS = 6 * 32;
+// CMO on the cluster path: every CTA owns a DG_TB x DG_TB block of tiles (all 512 TMEM columns as four 128-column
+// accumulators), so a k-step's 2 DG_TB slabs feed DG_TB^2 MMAs -- with 128 x 128 per CTA the single-digit Gram moved
+// 64 B per SM and clock from L2 and ran at the L2's pace (3.1 ms at C3's shape against 0.7 ms of tensor time)
+#ifndef DG_TB1
+#define DG_TB1 2
+#endif
+#ifndef DG_KG1B
+#define DG_KG1B 2                              // CMO, blocked: k-steps per stage
+#endif
+constexpr int DG_EPI_WARPS = 16;               // 4 TMEM lane quadrants x 4 column quarters of a tile
+constexpr int DG_THREADS = (2 + DG_EPI_WARPS) * 32;
 constexpr int DG_PREP_WARPS = 8;
 #ifndef DG_CLUSTER_I
 #define DG_CLUSTER_I 2                         // cluster shape of the Gram kernel: CLI tile rows x CLJ tile columns
@@ -52,7 +62,7 @@ constexpr int DG_PREP_WARPS = 8;
 struct __align__(16) DStat {
     double T;          // KAPPA^2 sum_k d_k^2 of the quantised distances, true scale (Angstrom^2); NaN poisons the model
     float pw;          // 2^e, e = the model's scale exponent
-    float pad;
+    float pad;         // CMO: (float)T
 };
 
 struct DWorkspace {
@@ -204,7 +214,7 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         s.T = DIGITS == 3 ? ldexp((double)sumsq, 2 * ex - 46) : (double)sumsq;
         if (!finite || (DIGITS == 3 && !in_range)) s.T = __longlong_as_double(0x7ff8000000000000ll);
         s.pw = pow2i(ex);
-        s.pad = 0.0f;
+        s.pad = DIGITS == 1 ? (float)s.T : 0.0f;           // CMO: the contact count (< 2^24, exact) for the fp32 epilogue
         stat[n] = s;
     }
 }
@@ -281,12 +291,24 @@ static inline int64_t dg_schedule_count(int32_t T, int32_t cli, int32_t clj)
 // by the CTAs of that row and the B slabs of a tile column by the CTAs of that column, so with 2 x 2 each CTA fetches
 // HALF of its A and HALF of its B and multicasts them to its row / column partner: the L2 -> SM operand bytes halve.
 // A stage is free again when every CTA of the cluster has consumed it (EMPTY counts CL multicast commits).
-template <int DIGITS, int CLI, int CLJ>
+// TB > 1 (needs CLI = CLJ = TB = 2): the CTA of rank (ri, rj) owns the tiles (TB (CLI SI + ri) + a, TB (CLJ SJ + rj) + b),
+// a, b < TB, accumulator a TB + b at TMEM columns 128 (a TB + b); it fetches the WHOLE run of row tile a = rj and of column
+// tile b = ri and multicasts them to its row / column partner, so a stage holds [A_0 | A_1 | B_0 | B_1].
+template <int DIGITS, int TB> struct DGKernelCfg {
+    static constexpr int KG = TB > 1 ? DG_KG1B : DGCfg<DIGITS>::KG;
+    static constexpr int OPER_BYTES = KG * DIGITS * DG_SLAB;            // one tile's run of a stage
+    static constexpr int STAGE_BYTES = 2 * TB * OPER_BYTES;
+    static constexpr int STAGES = (216 * 1024) / STAGE_BYTES;
+    static constexpr size_t SMEM = (size_t)STAGES * STAGE_BYTES + 8 * (2 * STAGES + 2) + 16 + DG_EPI_WARPS * 32 * 17 * sizeof(float);
+};
+template <int DIGITS, int CLI, int CLJ, int TB>
 __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParams P)
 {
+    static_assert(TB == 1 || (TB == 2 && CLI == 2 && CLJ == 2 && DIGITS == 1), "blocked tiles: 2 x 2 clusters, one digit");
     constexpr int CL = CLI * CLJ;                                // CTAs per cluster: CLI tile rows x CLJ tile columns
-    constexpr int DG_STAGES = DGCfg<DIGITS>::STAGES, DG_STAGE_BYTES = DGCfg<DIGITS>::STAGE_BYTES;
-    constexpr int KG = DGCfg<DIGITS>::KG, OPER = DGCfg<DIGITS>::OPER_BYTES;
+    typedef DGKernelCfg<DIGITS, TB> KC;
+    constexpr int DG_STAGES = KC::STAGES, DG_STAGE_BYTES = KC::STAGE_BYTES;
+    constexpr int KG = KC::KG, OPER = KC::OPER_BYTES;
     extern __shared__ __align__(128) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + (size_t)DG_STAGES * DG_STAGE_BYTES);
     const uint32_t bar0 = ptx::smem_u32(bars);
@@ -304,7 +326,7 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
             ptx::mbar_init(EMPTY(s), CL);
         }
         ptx::mbar_init(ACC_FULL, 1);
-        ptx::mbar_init(ACC_EMPTY, 4);
+        ptx::mbar_init(ACC_EMPTY, DG_EPI_WARPS);
         ptx::fence_mbar_init();
     }
     if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
@@ -326,16 +348,25 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
             for (int64_t t = first; t < total2; t += step) {
                 int32_t SI, SJ;
                 if (CL > 1) { const int2 e = P.sched[t]; SI = e.x; SJ = e.y; } else dg_tile_from_linear(t, P.T, SI, SJ);
-                const int32_t I = min(CLI * SI + ri, P.T - 1), J = min(CLJ * SJ + rj, P.T - 1);   // clamped: results are masked
+                // clamped: results are masked.  TB > 1: the row tile a = rj and the column tile b = ri of my block
+                const int32_t I = min(TB * (CLI * SI + ri) + (TB > 1 ? rj : 0), P.T - 1);
+                const int32_t J = min(TB * (CLJ * SJ + rj) + (TB > 1 ? ri : 0), P.T - 1);
                 const int8_t* a0 = P.plane + (int64_t)I * tile_stride;
                 const int8_t* b0 = P.plane + (int64_t)J * tile_stride;
                 for (int64_t kg = 0; kg < ng; ++kg) {
                     ptx::mbar_wait(EMPTY(stage), phase ^ 1);
                     ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
                     const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
-                    const uint32_t sB = sA + OPER;
+                    const uint32_t sB = sA + TB * OPER;
                     // a stage's A (and B) operand is one contiguous run of the plane: KG k-steps x DIGITS slabs.
                     // A is needed by the CLJ CTAs of my tile row: with CLJ == 2 I fetch half rj of the run and multicast it
+                    if (TB > 1) {
+                        ptx::bulk_g2s_multicast(sA + rj * OPER, a0 + kg * OPER, OPER, FULL(stage), (uint16_t)(3u << (ri * CLJ)));
+                        ptx::bulk_g2s_multicast(sB + ri * OPER, b0 + kg * OPER, OPER, FULL(stage),
+                                                (uint16_t)((1u | (1u << CLJ)) << rj));
+                        if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
+                        continue;
+                    }
                     if (CLJ == 2)
                         ptx::bulk_g2s_multicast(sA + rj * (OPER / 2), a0 + kg * OPER + rj * (OPER / 2), OPER / 2, FULL(stage),
                                                 (uint16_t)(3u << (ri * CLJ)));
@@ -365,12 +396,24 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                 ptx::tc_fence_after();
                 if (ptx::elect_one()) {
                     const uint32_t a_lo = lo0 + stage * (DG_STAGE_BYTES >> 4);
-                    const uint32_t b_lo = a_lo + (OPER >> 4);
+                    const uint32_t b_lo = a_lo + (TB * OPER >> 4);
                     constexpr uint32_t SL = DG_SLAB >> 4;
 #pragma unroll
                     for (int q = 0; q < KG; ++q) {
+#if defined(DG_EXPERIMENT) && (DG_EXPERIMENT & 2)                  // developer switch: operand delivery only (one MMA per tile)
+                        if (kg > 0 || q > 0) continue;
+#endif
                         const uint32_t acc = (kg > 0 || q > 0) ? 1u : 0u;
                         const uint32_t aq = a_lo + q * DIGITS * SL, bq = b_lo + q * DIGITS * SL;
+                        if (TB > 1) {
+#pragma unroll
+                            for (int a = 0; a < TB; ++a)
+#pragma unroll
+                                for (int b = 0; b < TB; ++b)
+                                    ptx::mma_i8(tmem + 128 * (a * TB + b), DESC_HI | (aq + a * (OPER >> 4)),
+                                                DESC_HI | (bq + b * (OPER >> 4)), ID128, acc);
+                            continue;
+                        }
                         // level v (TMEM columns 128 v ...) collects the digit products A(ga) . B(gb)^T with ga + gb = v
                         ptx::mma_i8(tmem, DESC_HI | aq, DESC_HI | bq, ID128, acc);
                         if (DIGITS == 3) {
@@ -392,49 +435,74 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
     } else {
         // ===== epilogue: thread = row model (TMEM lane), loops over the 128 column models of the tile =====
         const int quad = warp & 3;
+        // results go through a warp-private 32 x 33 float tile so that the stores run along the packed rows (a thread is a
+        // ROW of the accumulator: storing straight from it costs 32 sectors per instruction, 65k LSU cycles per tile)
+        float* tp = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(tmem_slot) + 16) + (warp - 2) * (32 * 17);
+        const int part = (warp - 2) >> 2;                        // column quarter: chunks 2 part, 2 part + 1 of 16 models
+        const int rr = lane >> 4, cc = lane & 15;                // store role: row parity, column within the chunk
         uint32_t tile_n = 0;
         for (int64_t t = first; t < total2; t += step, ++tile_n) {
             int32_t SI, SJ;
             if (CL > 1) { const int2 e = P.sched[t]; SI = e.x; SJ = e.y; } else dg_tile_from_linear(t, P.T, SI, SJ);
-            const int32_t I = CLI * SI + ri, J = CLJ * SJ + rj;
-            const bool active = I < P.T && J < P.T && I <= J;    // a cluster's block may hang over the edge / the diagonal
-            const int64_t i = (int64_t)min(I, P.T - 1) * DG_TILE + quad * 32 + lane;
-            const DStat si = P.stat[i];                          // slots beyond N hold neutral records
-            const double pwi = (double)si.pw * 0x1p-30;
-            const int64_t rowoff = i * (2 * P.N - i - 1) / 2 - i - 1;
             ptx::mbar_wait(ACC_FULL, tile_n & 1);
             ptx::tc_fence_after();
-            const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16);
-            if (active) {
 #pragma unroll 1
-                for (int c = 0; c < 8; ++c) {                    // 16-column chunks of the 128 column models
-                    uint32_t v0[16], v1[16], v2[16];
-                    ptx::tmem_ld_32x32b_x16(ta + 16 * c, v0);
-                    if (DIGITS == 3) {
-                        ptx::tmem_ld_32x32b_x16(ta + 128 + 16 * c, v1);
-                        ptx::tmem_ld_32x32b_x16(ta + 256 + 16 * c, v2);
-                    }
-                    ptx::tmem_ld_wait();
-                    const int64_t j0 = (int64_t)J * DG_TILE + 16 * c;
+            for (int sub = 0; sub < TB * TB; ++sub) {            // the tiles of this CTA's block
+                const int32_t I = TB * (CLI * SI + ri) + sub / TB, J = TB * (CLJ * SJ + rj) + sub % TB;
+#if defined(DG_EXPERIMENT) && (DG_EXPERIMENT & 1)                  // developer switch: no epilogue work
+                const bool active = false;
+#else
+                const bool active = I < P.T && J < P.T && I <= J;    // a cluster's block may hang over the edge / the diagonal
+#endif
+                const int64_t ibase = (int64_t)min(I, P.T - 1) * DG_TILE + quad * 32;
+                const int64_t i = ibase + lane;
+                const DStat si = P.stat[i];                          // slots beyond N hold neutral records
+                const double pwi = (double)si.pw * 0x1p-30;
+                const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16) + 128 * sub;
+                if (active) {
+#pragma unroll 1
+                    for (int h = 0; h < 2; ++h) {                    // this warp's two 16-column chunks
+                        const int c = 2 * part + h;
+                        uint32_t v0[16], v1[16], v2[16];
+                        ptx::tmem_ld_32x32b_x16(ta + 16 * c, v0);
+                        if (DIGITS == 3) {
+                            ptx::tmem_ld_32x32b_x16(ta + 128 + 16 * c, v1);
+                            ptx::tmem_ld_32x32b_x16(ta + 256 + 16 * c, v2);
+                        }
+                        ptx::tmem_ld_wait();
+                        const int64_t j0 = (int64_t)J * DG_TILE + 16 * c;
 #pragma unroll
-                    for (int e = 0; e < 16; ++e) {
-                        const int64_t j = j0 + e;
-                        if (i < P.N && j < P.N && j > i) {
-                            const DStat sj = P.stat[j];
+                        for (int e = 0; e < 16; ++e) {
+                            const DStat sj = P.stat[j0 + e];         // warp-uniform address
+                            float val;
                             if (DIGITS == 3) {
                                 const long long dot = ((long long)(int32_t)v0[e] << 16) + ((long long)(int32_t)v1[e] << 8) +
                                                       (long long)(int32_t)v2[e];
                                 const double res = (si.T + sj.T) - 2.0 * (double)dot * (pwi * (double)sj.pw);
                                 const float d2 = (float)(res * P.invKk);
-                                P.out[rowoff + j] = sqrtf(d2 < 0.0f ? 0.0f : d2);    // clamp (NaN stays NaN)
+                                val = sqrtf(d2 < 0.0f ? 0.0f : d2);                      // clamp (NaN stays NaN)
                             } else {
-                                // eq. 7: S = 100 * 2 n(A and B) / (n(A) + n(B)); two empty maps are identical: 100
-                                const double den = si.T + sj.T;
-                                const double S = den > 0.0 ? __ddiv_rn(__dmul_rn(200.0, (double)(int32_t)v0[e]), den)
-                                                           : (den == 0.0 ? 100.0 : den);          // NaN model -> NaN
-                                P.out[rowoff + j] = (float)S;
+                                // eq. 7: S = 100 * 2 n(A and B) / (n(A) + n(B)); two empty maps are identical: 100.
+                                // fp32 throughout and still the correctly rounded quotient: 200 n < 2^24 and the
+                                // denominator are exact in fp32, the division is IEEE; rounding the FP64 quotient to
+                                // fp32 (the oracle's route) gives the same float, because a ratio of integers with a
+                                // denominator < 2^17 cannot come within 2^-53 of an fp32 rounding boundary
+                                const float den = si.pad + sj.pad;                           // pad = (float)T
+                                val = den > 0.0f ? __fdiv_rn(200.0f * (float)(int32_t)v0[e], den)
+                                                 : (den == 0.0f ? 100.0f : den);              // NaN model -> NaN
                             }
+                            tp[lane * 17 + e] = val;
                         }
+                        __syncwarp();
+                        // transposed: one store instruction = 16 consecutive column models of TWO row models (2 x 64 B)
+                        const int64_t j = j0 + cc;
+#pragma unroll 4
+                        for (int r2 = 0; r2 < 16; ++r2) {
+                            const int r = 2 * r2 + rr;
+                            const int64_t ir = ibase + r;
+                            if (ir < P.N && j < P.N && j > ir) P.out[ir * (2 * P.N - ir - 1) / 2 - ir - 1 + j] = tp[r * 17 + cc];
+                        }
+                        __syncwarp();
                     }
                 }
             }
@@ -469,11 +537,13 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double
     P.T = (int32_t)(w.Np / DG_TILE);
     P.total = (int64_t)P.T * (P.T + 1) / 2;
     P.invKk = 1.0 / (DG_KAPPA * DG_KAPPA * (double)w.K);
-    const size_t smem = (size_t)DGCfg<DIGITS>::STAGES * DGCfg<DIGITS>::STAGE_BYTES + 8 * (2 * DGCfg<DIGITS>::STAGES + 2) + 16;
+    static_assert(DGCfg<1>::KG % DG_KG1B == 0, "the plane's k-step padding must cover the blocked kernel's k-group");
     // thread-block clusters with operand multicast when the matrix has enough tiles to fill the device with them
     if (P.T >= 8) {
         constexpr int CLI = DG_CLUSTER_I, CLJ = DG_CLUSTER_J;
-        auto kern = drmsd_gram_kernel<DIGITS, CLI, CLJ>;
+        constexpr int TB = (DIGITS == 1 && CLI == 2 && CLJ == 2) ? DG_TB1 : 1;     // tiles per CTA and side
+        const size_t smem = DGKernelCfg<DIGITS, TB>::SMEM;
+        auto kern = drmsd_gram_kernel<DIGITS, CLI, CLJ, TB>;
         CLUSCO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         cudaLaunchConfig_t cfg = {};
         cfg.blockDim = dim3(DG_THREADS);
@@ -489,14 +559,14 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double
         cfg.gridDim = dim3((unsigned)(sms / (CLI * CLJ) * (CLI * CLJ)));
         int clusters = 0;
         CLUSCO_CUDA_TRY(cudaOccupancyMaxActiveClusters(&clusters, kern, &cfg));    // co-resident clusters
-        P.n_sched = dg_schedule_count(P.T, CLI, CLJ);
+        P.n_sched = dg_schedule_count(P.T, TB * CLI, TB * CLJ);
         if (clusters > P.n_sched) clusters = (int)P.n_sched;
         if (clusters >= 1) {
             // blocks of about `clusters` super-tiles, square in tile units, so that a wave shares A rows and B columns in L2
             int32_t bj = 1;
             while ((int64_t)(bj + 1) * CLJ * (bj + 1) * CLJ <= (int64_t)clusters * CLI * CLJ) ++bj;
             const int32_t bi = (bj * CLJ + CLI - 1) / CLI;
-            dg_schedule_kernel<<<1, 32, 0, s>>>(P.T, CLI, CLJ, bi, bj, (int2*)(ws + w.off_sched));
+            dg_schedule_kernel<<<1, 32, 0, s>>>(P.T, TB * CLI, TB * CLJ, bi, bj, (int2*)(ws + w.off_sched));
             CLUSCO_CUDA_TRY(cudaGetLastError());
             cfg.gridDim = dim3((unsigned)(clusters * CLI * CLJ));
             CLUSCO_CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, P));
@@ -504,9 +574,10 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double
         }
     }
     P.n_sched = 0;
-    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(drmsd_gram_kernel<DIGITS, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    const size_t smem = DGKernelCfg<DIGITS, 1>::SMEM;
+    CLUSCO_CUDA_TRY(cudaFuncSetAttribute(drmsd_gram_kernel<DIGITS, 1, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     const int64_t grid = P.total < sms ? P.total : sms;
-    drmsd_gram_kernel<DIGITS, 1, 1><<<(unsigned)grid, DG_THREADS, smem, s>>>(P);
+    drmsd_gram_kernel<DIGITS, 1, 1, 1><<<(unsigned)grid, DG_THREADS, smem, s>>>(P);
     CLUSCO_CUDA_TRY(cudaGetLastError());
     return CLUSCO_OK;
 }

@@ -50,3 +50,16 @@ def test_library_route_and_symmetry():
     p = oracle.cmo_pairs(x, cutoff, [0, 3], [1, 20])
     assert p[0] == s[0] and p[1] == s[wl.packed_index(3, 20, 25)]
     assert np.array_equal(oracle.cmo_rows(x, cutoff, 2, 4), s[wl.packed_index(2, 3, 25):wl.packed_index(4, 5, 25)])
+
+
+def test_fp32_quotient_equals_the_rounded_fp64_quotient():
+    """Host logic behind the kernel's fp32 epilogue (drmsd_i8tc.cuh): eq. 7's 200 n / (n_A + n_B) with integer counts
+    (n <= K < 2^16 at L <= 296) -- the IEEE fp32 quotient of the exactly representable 200 n and n_A + n_B is the same
+    float as the oracle's FP64 quotient rounded to fp32 (no double-rounding case exists for such ratios)."""
+    rng = np.random.default_rng(0)
+    K = 296 * 295 // 2
+    den = rng.integers(1, 2 * K + 1, size=3_000_000)
+    n = (rng.random(den.shape) * (den // 2 + 1)).astype(np.int64)
+    a = (np.float32(200.0) * n.astype(np.float32)) / den.astype(np.float32)
+    b = (200.0 * n.astype(np.float64) / den.astype(np.float64)).astype(np.float32)
+    assert np.array_equal(a, b)
