@@ -49,7 +49,7 @@ template <int DIGITS> struct DGCfg {
 #define DG_TB1 2
 #endif
 #ifndef DG_KG1B
-#define DG_KG1B 2                              // CMO, blocked: k-steps per stage
+#define DG_KG1B 4                              // CMO, blocked: k-steps per stage
 #endif
 constexpr int DG_EPI_WARPS = 16;               // 4 TMEM lane quadrants x 4 column quarters of a tile
 constexpr int DG_THREADS = (2 + DG_EPI_WARPS) * 32;
@@ -150,55 +150,70 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         for (int it = 0; it < 8 && s_star > 0.0 && sqrt(s_star) >= cutoff; ++it) s_star = nextafter(s_star, 0.0);
         for (int it = 0; it < 8 && sqrt(s_star) < cutoff; ++it) s_star = nextafter(s_star, 1.0e300);
     }
-    // one pass over the K entries: a warp covers 4 k-steps per trip, lane = (k-step sub, group j8 of 4 consecutive
-    // entries), so that the digit bytes of 4 entries leave as one 32-bit store per digit
+    const float s_lo = (float)(s_star * (1.0 - 3.0e-6)), s_hi = (float)(s_star * (1.0 + 3.0e-6));
+    // one pass over the K entries, 4 k-steps (128 entries) per trip.  Computing: lane = entry within the k-step, so the
+    // warp reads 32 CONSECUTIVE atoms j of a row (stride 3 words: no bank conflict; four entries per lane put the four
+    // lane groups on the same banks).  Storing: a 4 x 4 byte transpose within each group of four lanes hands lane
+    // (4 j8 + sub) the digit bytes of entries 4 j8 .. 4 j8 + 3 of k-step sub: one 32-bit store per digit.
     const int64_t t128 = n >> 7;
     const int g = (int)(n & 127) >> 3, r8 = (int)(n & 7);
-    const int sub = lane >> 3, j8 = lane & 7;
+    const int sub = lane & 3, j8 = lane >> 2;
+    const uint32_t sel1 = (lane & 1) ? 0x3715u : 0x6240u, sel2 = (lane & 2) ? 0x3276u : 0x5410u;
     int8_t* base = plane + (t128 * ks * DIGITS) * DG_SLAB + g * 256 + (j8 >> 2) * 128 + r8 * 16 + (j8 & 3) * 4;
     long long sumsq = 0ll;
-    int i = 0, pos = sub * 32 + 4 * j8;                          // entry k = (4 trip + sub) 32 + 4 j8: pair (i, i + 1 + pos)
-    for (int64_t kk0 = 0; kk0 < ks; kk0 += 4) {
-        const int64_t kk = kk0 + sub;
-        const int64_t k0 = kk * 32 + 4 * j8;
-        uint32_t w0 = 0u, w1 = 0u, w2 = 0u;
-        if (valid && k0 < K) {
-            while (pos >= L - 1 - i) { pos -= L - 1 - i; ++i; }
-            int ii = i, pp = pos;
+    uint32_t ncontact = 0u;
+    int ii = 0, jj = 1 + lane;                                   // entry k = 32 kk + lane: pair (ii, jj), ii < jj < L
+    const int K32 = valid ? (int)K : 0, ks32 = (int)ks;          // K < 2^16 (L <= 296)
+    for (int kk0 = 0; kk0 < ks32; kk0 += 4) {
+        uint32_t W0 = 0u, W1 = 0u, W2 = 0u;                      // byte s: this lane's entry of k-step kk0 + s
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                if (k0 + e < K) {
-                    if (pp >= L - 1 - ii) { pp -= L - 1 - ii; ++ii; }     // at most one row wrap per step (rows are non-empty here)
-                    const double s2 = dist2(ii, ii + 1 + pp);
-                    ++pp;
-                    if (DIGITS == 3) {
-                        // sqrt by the fp32 reciprocal square root + one FP64 Newton step: relative error ~1e-13, far
-                        // below the 2^-24 quantisation step (the IEEE double square root is ~40 instructions)
-                        const double rf = (double)rsqrtf((float)s2);
-                        const double d0 = s2 * rf;
-                        const double d = s2 > 0.0 ? fma(0.5 * rf, fma(-d0, d0, s2), d0) : 0.0;
-                        const int I = __double2int_rn(d * scale);
-                        const int g2 = (int)(int8_t)(I & 0xff);
-                        const int I1 = (I - g2) >> 8;
-                        const int g1 = (int)(int8_t)(I1 & 0xff);
-                        const int g0 = (I1 - g1) >> 8;
-                        // |d|^2 from the SAME three levels the Gram keeps (I^2 minus the two dropped low-order levels),
-                        // so that an identical pair cancels to exactly 0
-                        sumsq += (long long)I * (long long)I - (long long)(512 * g1 * g2 + g2 * g2);
-                        w0 |= (uint32_t)(g0 & 0xff) << (8 * e);
-                        w1 |= (uint32_t)(g1 & 0xff) << (8 * e);
-                        w2 |= (uint32_t)(g2 & 0xff) << (8 * e);
-                    } else {
-                        const uint32_t cbit = s2 < s_star ? 1u : 0u;
-                        sumsq += cbit;
-                        w0 |= cbit << (8 * e);
-                    }
+        for (int s4 = 0; s4 < 4; ++s4) {
+            const int k = (kk0 + s4) * 32 + lane;
+            if (k < K32) {
+                while (jj >= L) { jj += ii + 2 - L; ++ii; }      // next row(s): entry (ii, L + d) is entry (ii + 1, ii + 2 + d)
+                if (DIGITS == 3) {
+                    const double s2 = dist2(ii, jj);
+                    // sqrt by the fp32 reciprocal square root + one FP64 Newton step: relative error ~1e-13, far
+                    // below the 2^-24 quantisation step (the IEEE double square root is ~40 instructions)
+                    const double rf = (double)rsqrtf((float)s2);
+                    const double d0 = s2 * rf;
+                    const double d = s2 > 0.0 ? fma(0.5 * rf, fma(-d0, d0, s2), d0) : 0.0;
+                    const int I = __double2int_rn(d * scale);
+                    const int g2 = (int)(int8_t)(I & 0xff);
+                    const int I1 = (I - g2) >> 8;
+                    const int g1 = (int)(int8_t)(I1 & 0xff);
+                    const int g0 = (I1 - g1) >> 8;
+                    // |d|^2 from the SAME three levels the Gram keeps (I^2 minus the two dropped low-order levels),
+                    // so that an identical pair cancels to exactly 0
+                    sumsq += (long long)I * (long long)I - (long long)(512 * g1 * g2 + g2 * g2);
+                    W0 |= (uint32_t)(g0 & 0xff) << (8 * s4);
+                    W1 |= (uint32_t)(g1 & 0xff) << (8 * s4);
+                    W2 |= (uint32_t)(g2 & 0xff) << (8 * s4);
+                } else {
+                    // fp32 screen: each difference carries one rounding (relative 2^-24), so the fp32 squared distance
+                    // is within 3e-7 of the FP64 one; outside a 3e-6 band around the threshold the fp32 comparison
+                    // decides, inside it (about one entry in 10^5) the FP64 evaluation of eq. 6 does
+                    const float fx = x[3 * ii] - x[3 * jj], fy = x[3 * ii + 1] - x[3 * jj + 1], fz = x[3 * ii + 2] - x[3 * jj + 2];
+                    const float s2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
+                    uint32_t cbit;
+                    if (s2f < s_lo) cbit = 1u;
+                    else if (s2f > s_hi) cbit = 0u;
+                    else cbit = dist2(ii, jj) < s_star ? 1u : 0u;
+                    ncontact += cbit;
+                    W0 |= cbit << (8 * s4);
                 }
             }
-            pos += 128;
+            jj += 32;
         }
-        if (kk < ks) {
-            int8_t* p = base + kk * DIGITS * DG_SLAB;
+        // 4 x 4 byte transpose over the four lanes of a group: 1-byte blocks with lane ^ 1, then 2-byte blocks with lane ^ 2
+        auto tr4 = [&](uint32_t W) {
+            const uint32_t a = __byte_perm(W, __shfl_xor_sync(0xffffffffu, W, 1), sel1);
+            return __byte_perm(a, __shfl_xor_sync(0xffffffffu, a, 2), sel2);
+        };
+        const uint32_t w0 = tr4(W0), w1 = DIGITS == 3 ? tr4(W1) : 0u, w2 = DIGITS == 3 ? tr4(W2) : 0u;
+        const int kk = kk0 + sub;
+        if (kk < ks32) {
+            int8_t* p = base + (int64_t)kk * DIGITS * DG_SLAB;
             *reinterpret_cast<uint32_t*>(p) = w0;
             if (DIGITS == 3) {
                 *reinterpret_cast<uint32_t*>(p + DG_SLAB) = w1;
@@ -206,6 +221,7 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
             }
         }
     }
+    if (DIGITS == 1) sumsq = (long long)ncontact;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) sumsq += __shfl_xor_sync(0xffffffffu, sumsq, o);
     finite = __all_sync(0xffffffffu, finite);
