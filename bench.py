@@ -411,7 +411,7 @@ def drmsd_side(clusco, coords, out, flush, N, L, P, pk):
             "pairs_per_s": P / (ms * 1e-3),
             "roofline": {"bound": "tensor", "achieved": flops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",
                          "frac": flops / (ms * 1e-3) / 1e12 / peak,
-                         "issued_frac": issued / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel (+ drmsd_prep_kernel)",
+                         "issued_frac": issued / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel<3,2,2,1> (+ drmsd_prep_kernel<3>)",
                          "workspace_bytes": int(ws.numel())}}
 
 
@@ -440,7 +440,7 @@ def cmo_side(clusco, coords, out, flush, N, L, P, pk):
     return {"workload": f"CMO all-vs-all, cut-off 8 A, N={N} x L={L} (K={K} contact bits per model)", "ms": ms,
             "pairs_per_s": P / (ms * 1e-3),
             "roofline": {"bound": "tensor", "achieved": ops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TOP/s",
-                         "frac": ops / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel<1> (+ drmsd_prep_kernel<1>)",
+                         "frac": ops / (ms * 1e-3) / 1e12 / peak, "kernel": "drmsd_gram_kernel<1,2,2,2> (+ drmsd_prep_kernel<1>)",
                          "workspace_bytes": int(ws.numel())}}
 
 
