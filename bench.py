@@ -406,7 +406,7 @@ def drmsd_side(clusco, coords, out, flush, N, L, P, pk):
     peak = 2.0 * pk["bf16_tflops"]
     Np = (N + 127) // 128 * 128
     T = Np // 128
-    issued = 2.0 * (T * (T + 1) // 2) * ((K + 31) // 32) * 128 * (6 * 128) * 32        # six N=128 MMAs per k-step
+    issued = 2.0 * (T * (T + 1) // 2) * ((K + 31) // 32) * 128 * (6 * 128) * 32        # 2 x N=256 + 2 x N=128 MMAs per k-step (= six N=128 products)
     return {"workload": f"dRMSD all-vs-all, N={N} x L={L} (K={K} distances per model)", "ms": ms,
             "pairs_per_s": P / (ms * 1e-3),
             "roofline": {"bound": "tensor", "achieved": flops / (ms * 1e-3) / 1e12, "peak": peak, "unit": "TFLOP/s",

@@ -90,3 +90,20 @@ def test_cmo_cluster_path_every_pair(clusco, N, L):
     got = clusco.clusco_cmo_allpairs(_dev(x), 9.0).cpu().numpy()
     assert np.array_equal(got, want)
     assert want.min() < 90.0
+
+
+@pytest.mark.parametrize("scale,shift", [(1.0, 0.0), (1.0, 4096.0), (0.1, 0.0), (0.7, -333.0)])
+def test_cmo_distances_at_the_cutoff(clusco, scale, shift):
+    """The prepare kernel screens eq. 6 in fp32 and falls back to the FP64 evaluation inside a narrow band around the
+    cut-off: integer-lattice models have many pairs EXACTLY at the cut-off distance (3-4-0, 5-0-0, ...: strict
+    inequality -> no contact) and, scaled by a non-dyadic factor, many within a few ulp of it."""
+    rng = np.random.default_rng(17)
+    N, L = 150, 60
+    x = (rng.integers(0, 9, size=(N, L, 3)).astype(np.float64) * scale + shift).astype(np.float32)
+    cutoff = float(np.float32(5.0 * scale))
+    want = oracle.cmo_allpairs(x, cutoff).astype(np.float32)
+    got = clusco.clusco_cmo_allpairs(_dev(x), cutoff).cpu().numpy()
+    assert np.array_equal(got, want), np.abs(got - want).max()
+    ova_want = oracle.cmo_one_vs_all(x[0], x[1:], cutoff).astype(np.float32)
+    ova_got = clusco.clusco_cmo_one_vs_all(_dev(x[0]), _dev(x[1:]), cutoff).cpu().numpy()
+    assert np.array_equal(ova_got, ova_want)
