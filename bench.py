@@ -465,9 +465,22 @@ def gdt_side(clusco, wl):
     torch.cuda.synchronize()
     ms = sum(a.elapsed_time(b) for a, b in ev) / reps
     o = out.cpu().numpy()
+    # all-versus-all form on the first 200 of those models: 19 900 pairs, one warp per pair
+    M = 200
+    sub = coords[:M].contiguous()
+    ap = clusco.clusco_gdt_allpairs(sub)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    a.record(stream)
+    clusco.clusco_gdt_allpairs(sub, ap)
+    b.record(stream)
+    torch.cuda.synchronize()
+    ms_ap = a.elapsed_time(b)
     return {"workload": f"GDT_TS / TM-score / MaxSub, 1 native vs first {N} models of C5 (L=150)", "ms": ms,
             "models_per_s": N / (ms * 1e-3), "mean_gdt_ts": float(o[:, 0].mean()), "mean_tm_score": float(o[:, 1].mean()),
-            "kernel": "gdt_kernel<false>", "bound": "alu (FP64, data-dependent iteration count)"}
+            "kernel": "gdt_kernel<false>", "bound": "alu (FP64, data-dependent iteration count)",
+            "allpairs": {"workload": f"all-vs-all over the first {M} of those models ({M * (M - 1) // 2} pairs)", "ms": ms_ap,
+                         "pairs_per_s": M * (M - 1) // 2 / (ms_ap * 1e-3), "kernel": "gdt_kernel<true>"}}
 
 
 def launches_per_step(engine):

@@ -112,6 +112,34 @@ __device__ __forceinline__ double gdt_warp_sum(double v)
     return v;
 }
 
+// Sums of 16 values over the warp, every lane receiving all 16: a transposed butterfly -- at offset 16 a lane keeps one
+// half of the values and hands the other half to its partner, at offset 8 a quarter, ... -- so that 16 exchanges (plus 16
+// broadcasts) replace the 80 of sixteen separate butterflies.  Value e ends up on lanes 2 e and 2 e + 1.
+__device__ __forceinline__ void gdt_warp_sum16(double (&v)[16], int lane)
+{
+    const bool b4 = lane & 16, b3 = lane & 8, b2 = lane & 4, b1 = lane & 2;
+    double w8[8], w4[4], w2[2];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+        const double keep = b4 ? v[e + 8] : v[e], send = b4 ? v[e] : v[e + 8];
+        w8[e] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const double keep = b3 ? w8[e + 4] : w8[e], send = b3 ? w8[e] : w8[e + 4];
+        w4[e] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+        const double keep = b2 ? w4[e + 2] : w4[e], send = b2 ? w4[e] : w4[e + 2];
+        w2[e] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    double w1 = (b1 ? w2[1] : w2[0]) + __shfl_xor_sync(0xffffffffu, b1 ? w2[0] : w2[1], 2);
+    w1 += __shfl_xor_sync(0xffffffffu, w1, 1);
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = __shfl_sync(0xffffffffu, w1, 2 * e);
+}
+
 // centre a model (FP64) into shared memory, one warp; returns whether all its coordinates are finite
 __device__ __forceinline__ bool gdt_load_centred(double* __restrict__ dst, const float* __restrict__ x, int L, int lane)
 {
@@ -209,11 +237,15 @@ __global__ void __launch_bounds__(GDT_WARPS * 32) gdt_kernel(const float* __rest
                             S[3] += b1 * a0; S[4] += b1 * a1; S[5] += b1 * a2;
                             S[6] += b2 * a0; S[7] += b2 * a1; S[8] += b2 * a2;
                         }
-                    cnt = gdt_warp_sum(cnt);
-                    ca0 = gdt_warp_sum(ca0) / cnt; ca1 = gdt_warp_sum(ca1) / cnt; ca2 = gdt_warp_sum(ca2) / cnt;
-                    cb0 = gdt_warp_sum(cb0) / cnt; cb1 = gdt_warp_sum(cb1) / cnt; cb2 = gdt_warp_sum(cb2) / cnt;
+                    {
+                        double v[16] = {cnt, ca0, ca1, ca2, cb0, cb1, cb2, S[0], S[1], S[2], S[3], S[4], S[5], S[6], S[7], S[8]};
+                        gdt_warp_sum16(v, lane);
+                        cnt = v[0];
+                        ca0 = v[1] / cnt; ca1 = v[2] / cnt; ca2 = v[3] / cnt;
+                        cb0 = v[4] / cnt; cb1 = v[5] / cnt; cb2 = v[6] / cnt;
 #pragma unroll
-                    for (int e = 0; e < 9; ++e) S[e] = gdt_warp_sum(S[e]);
+                        for (int e = 0; e < 9; ++e) S[e] = v[7 + e];
+                    }
                     // centre the cross-covariance on the selection: S - n cb ca^T
                     S[0] -= cnt * cb0 * ca0; S[1] -= cnt * cb0 * ca1; S[2] -= cnt * cb0 * ca2;
                     S[3] -= cnt * cb1 * ca0; S[4] -= cnt * cb1 * ca1; S[5] -= cnt * cb1 * ca2;
