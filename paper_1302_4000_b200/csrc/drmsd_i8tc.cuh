@@ -45,9 +45,6 @@ template <int DIGITS> struct DGCfg {
 // CMO on the cluster path: every CTA owns a DG_TB x DG_TB block of tiles (all 512 TMEM columns as four 128-column
 // accumulators), so a k-step's 2 DG_TB slabs feed DG_TB^2 MMAs -- with 128 x 128 per CTA the single-digit Gram moved
 // 64 B per SM and clock from L2 and ran at the L2's pace (3.1 ms at C3's shape against 0.7 ms of tensor time)
-#ifndef DG_TB1
-#define DG_TB1 2
-#endif
 #ifndef DG_KG1B
 #define DG_KG1B 4                              // CMO, blocked: k-steps per stage
 #endif
@@ -73,7 +70,7 @@ static inline DWorkspace drmsd_workspace_layout(int64_t N, int32_t L, int digits
 {
     DWorkspace w;
     w.N = N;
-    w.Np = round_up(N, DG_TILE);
+    w.Np = round_up(N, digits == 1 ? 2 * DG_TILE : DG_TILE);   // CMO: 256-row plane tiles (two slabs per k-step)
     w.K = (int64_t)L * (L - 1) / 2;
     const int64_t kg = digits == 3 ? DGCfg<3>::KG : DGCfg<1>::KG;
     w.ks = round_up((w.K + 31) / 32, kg);
@@ -159,7 +156,11 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
     const int g = (int)(n & 127) >> 3, r8 = (int)(n & 7);
     const int sub = lane & 3, j8 = lane >> 2;
     const uint32_t sel1 = (lane & 1) ? 0x3715u : 0x6240u, sel2 = (lane & 2) ? 0x3276u : 0x5410u;
-    int8_t* base = plane + (t128 * ks * DIGITS) * DG_SLAB + g * 256 + (j8 >> 2) * 128 + r8 * 16 + (j8 & 3) * 4;
+    // DIGITS = 3: P[tile128][k-step][digit][4 KB].  DIGITS = 1: P[tile256][k-step][half][4 KB] -- the two 128-row slabs of a
+    // k-step are consecutive, so a 256-model tile is ONE N = 256 operand and either half is an M = 128 operand
+    constexpr int64_t KSTEP_SLABS = DIGITS == 3 ? 3 : 2;
+    int8_t* base = plane + (DIGITS == 3 ? t128 * ks * 3 : (t128 >> 1) * ks * 2 + (t128 & 1)) * DG_SLAB + g * 256 +
+                   (j8 >> 2) * 128 + r8 * 16 + (j8 & 3) * 4;
     long long sumsq = 0ll;
     uint32_t ncontact = 0u;
     int ii = 0, jj = 1 + lane;                                   // entry k = 32 kk + lane: pair (ii, jj), ii < jj < L
@@ -212,7 +213,7 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         const uint32_t w0 = tr4(W0), w1 = DIGITS == 3 ? tr4(W1) : 0u, w2 = DIGITS == 3 ? tr4(W2) : 0u;
         const int kk = kk0 + sub;
         if (kk < ks32) {
-            int8_t* p = base + (int64_t)kk * DIGITS * DG_SLAB;
+            int8_t* p = base + (int64_t)kk * KSTEP_SLABS * DG_SLAB;
             *reinterpret_cast<uint32_t*>(p) = w0;
             if (DIGITS == 3) {
                 *reinterpret_cast<uint32_t*>(p + DG_SLAB) = w1;
@@ -320,6 +321,7 @@ template <int DIGITS, int CLI, int CLJ, int TB>
 __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParams P)
 {
     static_assert(TB == 1 || (TB == 2 && CLI == 2 && CLJ == 2 && DIGITS == 1), "blocked tiles: 2 x 2 clusters, one digit");
+    static_assert(DIGITS == 3 || TB == 2 || CLI * CLJ == 1, "one digit: 256-row plane tiles need the blocked kernel or no cluster");
     constexpr int CL = CLI * CLJ;                                // CTAs per cluster: CLI tile rows x CLJ tile columns
     typedef DGKernelCfg<DIGITS, TB> KC;
     constexpr int DG_STAGES = KC::STAGES, DG_STAGE_BYTES = KC::STAGE_BYTES;
@@ -359,29 +361,56 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
         // ===== producer =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0;
-            const int64_t tile_stride = P.ks * DIGITS * DG_SLAB;
+            const int64_t tile_stride = P.ks * (DIGITS == 3 ? 3 : 2) * DG_SLAB;     // DIGITS = 1: stride of a 256-row tile
             for (int64_t t = first; t < total2; t += step) {
                 int32_t SI, SJ;
                 if (CL > 1) { const int2 e = P.sched[t]; SI = e.x; SJ = e.y; } else dg_tile_from_linear(t, P.T, SI, SJ);
-                // clamped: results are masked.  TB > 1: the row tile a = rj and the column tile b = ri of my block
-                const int32_t I = min(TB * (CLI * SI + ri) + (TB > 1 ? rj : 0), P.T - 1);
-                const int32_t J = min(TB * (CLJ * SJ + rj) + (TB > 1 ? ri : 0), P.T - 1);
+                if (TB > 1) {
+                    // my block = the 256-row tile CLI SI + ri times the 256-row tile CLJ SJ + rj (clamped: results are
+                    // masked); a stage's A (B) operand is ONE contiguous run of that tile, KG k-steps x [half 0 | half 1]:
+                    // I fetch half rj (ri) of the run -- KG / 2 k-steps -- and multicast it to my row (column) partner
+                    const int32_t IR = min(CLI * SI + ri, P.T / 2 - 1), JC = min(CLJ * SJ + rj, P.T / 2 - 1);
+                    const int8_t* a0 = P.plane + (int64_t)IR * tile_stride + rj * OPER;
+                    const int8_t* b0 = P.plane + (int64_t)JC * tile_stride + ri * OPER;
+                    for (int64_t kg = 0; kg < ng; ++kg) {
+                        ptx::mbar_wait(EMPTY(stage), phase ^ 1);
+                        ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
+                        const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
+                        const uint32_t sB = sA + TB * OPER;
+                        ptx::bulk_g2s_multicast(sA + rj * OPER, a0 + kg * 2 * OPER, OPER, FULL(stage), (uint16_t)(3u << (ri * CLJ)));
+                        ptx::bulk_g2s_multicast(sB + ri * OPER, b0 + kg * 2 * OPER, OPER, FULL(stage),
+                                                (uint16_t)((1u | (1u << CLJ)) << rj));
+                        if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
+                    }
+                    continue;
+                }
+                const int32_t I = min(CLI * SI + ri, P.T - 1), J = min(CLJ * SJ + rj, P.T - 1);   // clamped: results are masked
+                if (DIGITS == 1) {
+                    // one digit, no clusters (small N): the 128-row halves of the 256-row plane tiles, one 4 KB slab per k-step
+                    const int8_t* a0 = P.plane + (int64_t)(I >> 1) * tile_stride + (I & 1) * DG_SLAB;
+                    const int8_t* b0 = P.plane + (int64_t)(J >> 1) * tile_stride + (J & 1) * DG_SLAB;
+                    for (int64_t kg = 0; kg < ng; ++kg) {
+                        ptx::mbar_wait(EMPTY(stage), phase ^ 1);
+                        ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
+                        const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
+                        const uint32_t sB = sA + OPER;
+                        for (int q = 0; q < KG; ++q) {
+                            ptx::bulk_g2s(sA + q * DG_SLAB, a0 + (kg * KG + q) * 2 * DG_SLAB, DG_SLAB, FULL(stage));
+                            ptx::bulk_g2s(sB + q * DG_SLAB, b0 + (kg * KG + q) * 2 * DG_SLAB, DG_SLAB, FULL(stage));
+                        }
+                        if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
+                    }
+                    continue;
+                }
                 const int8_t* a0 = P.plane + (int64_t)I * tile_stride;
                 const int8_t* b0 = P.plane + (int64_t)J * tile_stride;
                 for (int64_t kg = 0; kg < ng; ++kg) {
                     ptx::mbar_wait(EMPTY(stage), phase ^ 1);
                     ptx::mbar_expect_tx(FULL(stage), DG_STAGE_BYTES);
                     const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
-                    const uint32_t sB = sA + TB * OPER;
+                    const uint32_t sB = sA + OPER;
                     // a stage's A (and B) operand is one contiguous run of the plane: KG k-steps x DIGITS slabs.
                     // A is needed by the CLJ CTAs of my tile row: with CLJ == 2 I fetch half rj of the run and multicast it
-                    if (TB > 1) {
-                        ptx::bulk_g2s_multicast(sA + rj * OPER, a0 + kg * OPER, OPER, FULL(stage), (uint16_t)(3u << (ri * CLJ)));
-                        ptx::bulk_g2s_multicast(sB + ri * OPER, b0 + kg * OPER, OPER, FULL(stage),
-                                                (uint16_t)((1u | (1u << CLJ)) << rj));
-                        if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
-                        continue;
-                    }
                     if (CLJ == 2)
                         ptx::bulk_g2s_multicast(sA + rj * (OPER / 2), a0 + kg * OPER + rj * (OPER / 2), OPER / 2, FULL(stage),
                                                 (uint16_t)(3u << (ri * CLJ)));
@@ -421,12 +450,11 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                         const uint32_t acc = (kg > 0 || q > 0) ? 1u : 0u;
                         const uint32_t aq = a_lo + q * DIGITS * SL, bq = b_lo + q * DIGITS * SL;
                         if (TB > 1) {
+                            // k-step q of the A run = [rows 0..127 | rows 128..255]; of the B run = one N = 256 operand:
+                            // accumulator a TB + b = TMEM columns 256 a + 128 b
 #pragma unroll
                             for (int a = 0; a < TB; ++a)
-#pragma unroll
-                                for (int b = 0; b < TB; ++b)
-                                    ptx::mma_i8(tmem + 128 * (a * TB + b), DESC_HI | (aq + a * (OPER >> 4)),
-                                                DESC_HI | (bq + b * (OPER >> 4)), ID128, acc);
+                                ptx::mma_i8(tmem + 256 * a, DESC_HI | (a_lo + (2 * q + a) * SL), DESC_HI | (b_lo + 2 * q * SL), ID256, acc);
                             continue;
                         }
                         // level v (TMEM columns 128 v ...) collects the digit products A(ga) . B(gb)^T with ga + gb = v
@@ -560,7 +588,7 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double
     // thread-block clusters with operand multicast when the matrix has enough tiles to fill the device with them
     if (P.T >= 8) {
         constexpr int CLI = DG_CLUSTER_I, CLJ = DG_CLUSTER_J;
-        constexpr int TB = (DIGITS == 1 && CLI == 2 && CLJ == 2) ? DG_TB1 : 1;     // tiles per CTA and side
+        constexpr int TB = DIGITS == 1 ? 2 : 1;                                      // tiles per CTA and side
         const size_t smem = DGKernelCfg<DIGITS, TB>::SMEM;
         auto kern = drmsd_gram_kernel<DIGITS, CLI, CLJ, TB>;
         CLUSCO_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
