@@ -80,7 +80,7 @@ def test_cmo_full_size_sampled(clusco):
     assert np.array_equal(got[wl.packed_index(pi, pj, ens.N)], want)
 
 
-@pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12)])
+@pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12), (2049, 20)])
 def test_cmo_cluster_path_every_pair(clusco, N, L):
     """N >= 897 takes the 2 x 2 cluster kernel with multicast operands (odd tile count: overhanging blocks)."""
     rng = np.random.default_rng(N + L)

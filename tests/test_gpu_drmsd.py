@@ -100,7 +100,7 @@ def test_drmsd_full_size_sampled(clusco):
     _check(got[wl.packed_index(pi, pj, ens.N)], d_ref, d2_ref, "C3 sampled")
 
 
-@pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12)])
+@pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12), (2049, 20)])
 def test_drmsd_cluster_path_every_pair(clusco, N, L):
     """N >= 897 (8 tiles per side) takes the 2 x 2 cluster kernel with multicast operands; T = 9 is odd, so the
     last cluster row / column hangs over the edge and the diagonal blocks hold one masked tile."""
