@@ -46,7 +46,7 @@ template <int DIGITS> struct DGCfg {
 // accumulators), so a k-step's 2 DG_TB slabs feed DG_TB^2 MMAs -- with 128 x 128 per CTA the single-digit Gram moved
 // 64 B per SM and clock from L2 and ran at the L2's pace (3.1 ms at C3's shape against 0.7 ms of tensor time)
 #ifndef DG_KG1B
-#define DG_KG1B 4                              // CMO, blocked: k-steps per stage
+#define DG_KG1B 2                              // CMO, blocked: k-steps per stage (measured: 2 -> 1.69 ms, 4 -> 1.71 ms whole call)
 #endif
 constexpr int DG_EPI_WARPS = 16;               // 4 TMEM lane quadrants x 4 column quarters of a tile
 constexpr int DG_THREADS = (2 + DG_EPI_WARPS) * 32;
@@ -543,11 +543,16 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                         __syncwarp();
                         // transposed: one store instruction = 16 consecutive column models of TWO row models (2 x 64 B)
                         const int64_t j = j0 + cc;
+                        // packed offset of row ir: ir (2N - ir - 1) / 2 - ir - 1; two rows further it grows by 2N - 2 ir - 5
+                        int64_t ir = ibase + rr;
+                        float* dst = P.out + (ir * (2 * P.N - ir - 1) / 2 - ir - 1 + j);
+                        int64_t inc = 2 * P.N - 2 * ir - 5;
 #pragma unroll 4
                         for (int r2 = 0; r2 < 16; ++r2) {
-                            const int r = 2 * r2 + rr;
-                            const int64_t ir = ibase + r;
-                            if (ir < P.N && j < P.N && j > ir) P.out[ir * (2 * P.N - ir - 1) / 2 - ir - 1 + j] = tp[r * 17 + cc];
+                            if (ir < P.N && j < P.N && j > ir) *dst = tp[(2 * r2 + rr) * 17 + cc];
+                            dst += inc;
+                            inc -= 4;
+                            ir += 2;
                         }
                         __syncwarp();
                     }
