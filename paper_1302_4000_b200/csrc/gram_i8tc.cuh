@@ -372,7 +372,10 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             float* dst;                          // out + rowoff + j0
             int32_t i, j0;                       // the pairs are (i, j0) and (i, j0 + 4)
             bool ok0, ok1;
-        } pend = {};
+        };
+        // two records used alternately (the loop below is unrolled by two tiles), so that handing a tile's invariants
+        // to the next iteration costs no register moves
+        Pending pendA = {}, pendB = {};
         bool have_pend = false;
         // ROWSTATS: running sum / count of the row this lane group is on (rows persist over consecutive tiles)
         double acc_sum = 0.0;
@@ -407,7 +410,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 if (acc_cnt) atomicAdd(P.sink.below + acc_i, acc_cnt);
             }
         };
-        auto finish_pending = [&]() {
+        auto finish_pending = [&](const Pending& pend) {
 #if defined(I8_EXPERIMENT) && (I8_EXPERIMENT == 1 || I8_EXPERIMENT >= 3)   // developer switch: no eq. 2 arithmetic
             const float2 c = make_float2(pend.inv.c2.x + pend.inv.c1.x + pend.Thi, pend.inv.c2.y + pend.inv.d.y + pend.Thj.y);
 #else
@@ -473,7 +476,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 }
             }
         };
-        for (uint32_t n = team; n < ntiles; n += 2) {
+        auto tile_body = [&](const uint32_t n, Pending& pend, const Pending& prev, const bool have_prev) {
             if (I != curI) {                                     // per-row quantities (warp-uniform branch)
                 curI = I;
                 i = I * I8_ROW_MODELS + quad * 8 + r;
@@ -494,7 +497,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
 #if defined(I8_EXPERIMENT) && I8_EXPERIMENT >= 3              // developer switch: no TMEM loads, no arithmetic
 #pragma unroll
             for (int q = 0; q < 9; ++q) m[q] = make_float2((float)(n + q), (float)(n + q + 1));
-            if (have_pend) finish_pending();
+            if (have_prev) finish_pending(prev);
 #else
             {
                 // levels 1 and 2 first: T = 2^8 V1 + V2 fits int32 (|T| < 2^31 for L <= 256 because |d0| <= 127)
@@ -506,7 +509,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                         ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 48 + 16 * q, v1[q][h]);
                         ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 96 + 16 * q, v2[q][h]);
                     }
-                if (have_pend) finish_pending();                 // previous tile's serial half, under the load latency
+                if (have_prev) finish_pending(prev);             // previous tile's serial half, under the load latency
                 ptx::tmem_ld_wait();
                 const float2 s30 = make_float2(0x1p-30f, 0x1p-30f);
 #pragma unroll
@@ -554,13 +557,23 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             pend.j0 = j0;
             pend.ok0 = row_ok && j0 < N32 && j0 > i;             // masked pairs are simply not stored
             pend.ok1 = row_ok && j0 + 4 < N32 && j0 + 4 > i;
-            have_pend = true;
             // advance two tiles
 #pragma unroll
             for (int s = 0; s < 2; ++s)
                 if (++J >= Tc32) { ++I; J = 2 * I; }
+        };
+        bool last_is_A = true;
+        for (uint32_t n = team; n < ntiles; n += 4) {
+            tile_body(n, pendA, pendB, have_pend);
+            have_pend = true;
+            last_is_A = true;
+            if (n + 2 >= ntiles) break;
+            tile_body(n + 2, pendB, pendA, true);
+            last_is_A = false;
         }
-        if (have_pend) finish_pending();
+        if (have_pend) {
+            if (last_is_A) finish_pending(pendA); else finish_pending(pendB);
+        }
         if (MODE == SINK_ROWSTATS) flush_row();
         if (MODE == SINK_BELOW) flush_hits();
     }
