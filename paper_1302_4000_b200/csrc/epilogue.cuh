@@ -137,12 +137,12 @@ __device__ __forceinline__ EPairT<V> eq2_energy(const EqInvariants<V> inv)
     using namespace lp;
     const V c2 = inv.c2, c1 = inv.c1, d = inv.d;
     // largest root of the cubic, Viete:  l1 = q + 2 sqrt(p) cos(acos(rr / p^1.5) / 3)
+    // with q = c2 / 3:  p = (c2^2 - 3 c1) / 9 = q^2 - c1 / 3,   r = (27 d^2 + c2 (2 c2^2 - 9 c1)) / 54 = d^2 / 2 + q (q^2 - c1 / 2)
     const V q = mul(c2, splat<V>(1.0f / 3.0f));
-    V pp = mul(fma(c2, c2, mul(splat<V>(-3.0f), c1)), splat<V>(1.0f / 9.0f));
+    V pp = fma(q, q, mul(c1, splat<V>(-1.0f / 3.0f)));
     pp = map(pp, [](float t) { return t > 0.0f ? t : 0.0f; });
     const V d2 = mul(d, d);
-    const V rr = mul(fma(splat<V>(27.0f), d2, mul(c2, fma(mul(splat<V>(2.0f), c2), c2, mul(splat<V>(-9.0f), c1)))),
-                     splat<V>(1.0f / 54.0f));
+    const V rr = fma(q, fma(q, q, mul(c1, splat<V>(-0.5f))), mul(d2, splat<V>(0.5f)));
     const V sp = map(pp, [](float t) { return sqrt_fast(t); });
     const V ps = mul(pp, sp);
     const V ratio = zip3(pp, rr, ps, [](float p_, float r_, float ps_) { return p_ > 0.0f ? r_ * rcp_fast(ps_) : 1.0f; });
