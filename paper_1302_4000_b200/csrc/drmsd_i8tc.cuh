@@ -45,6 +45,9 @@ template <int DIGITS> struct DGCfg {
 // CMO on the cluster path: every CTA owns a DG_TB x DG_TB block of tiles (all 512 TMEM columns as four 128-column
 // accumulators), so a k-step's 2 DG_TB slabs feed DG_TB^2 MMAs -- with 128 x 128 per CTA the single-digit Gram moved
 // 64 B per SM and clock from L2 and ran at the L2's pace (3.1 ms at C3's shape against 0.7 ms of tensor time)
+#ifndef DG_CMO_CLUSTER_I
+#define DG_CMO_CLUSTER_I 1                     // CMO cluster rows: 2 (2 x 2, 132 SMs) or 1 (1 x 2, all 148 SMs, 1.5 x the L2 reads)
+#endif
 #ifndef DG_KG1B
 #define DG_KG1B 2                              // CMO, blocked: k-steps per stage (measured: 2 -> 1.69 ms, 4 -> 1.71 ms whole call)
 #endif
@@ -320,7 +323,7 @@ template <int DIGITS, int TB> struct DGKernelCfg {
 template <int DIGITS, int CLI, int CLJ, int TB>
 __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParams P)
 {
-    static_assert(TB == 1 || (TB == 2 && CLI == 2 && CLJ == 2 && DIGITS == 1), "blocked tiles: 2 x 2 clusters, one digit");
+    static_assert(TB == 1 || (TB == 2 && CLI <= 2 && CLJ == 2 && DIGITS == 1), "blocked tiles: 2 x 2 or 1 x 2 clusters, one digit");
     static_assert(DIGITS == 3 || TB == 2 || CLI * CLJ == 1, "one digit: 256-row plane tiles need the blocked kernel or no cluster");
     constexpr int CL = CLI * CLJ;                                // CTAs per cluster: CLI tile rows x CLJ tile columns
     typedef DGKernelCfg<DIGITS, TB> KC;
@@ -378,8 +381,11 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                         const uint32_t sA = ptx::smem_u32(smem + (size_t)stage * DG_STAGE_BYTES);
                         const uint32_t sB = sA + TB * OPER;
                         ptx::bulk_g2s_multicast(sA + rj * OPER, a0 + kg * 2 * OPER, OPER, FULL(stage), (uint16_t)(3u << (ri * CLJ)));
-                        ptx::bulk_g2s_multicast(sB + ri * OPER, b0 + kg * 2 * OPER, OPER, FULL(stage),
-                                                (uint16_t)((1u | (1u << CLJ)) << rj));
+                        if (CLI == 2)
+                            ptx::bulk_g2s_multicast(sB + ri * OPER, b0 + kg * 2 * OPER, OPER, FULL(stage),
+                                                    (uint16_t)((1u | (1u << CLJ)) << rj));
+                        else
+                            ptx::bulk_g2s(sB, b0 + kg * 2 * OPER, 2 * OPER, FULL(stage));     // 1 x 2 cluster: my own column tile
                         if (++stage == DG_STAGES) { stage = 0; phase ^= 1; }
                     }
                     continue;
@@ -592,7 +598,7 @@ static inline int drmsd_launch(const float* coords, int64_t N, int32_t L, double
     static_assert(DGCfg<1>::KG % DG_KG1B == 0, "the plane's k-step padding must cover the blocked kernel's k-group");
     // thread-block clusters with operand multicast when the matrix has enough tiles to fill the device with them
     if (P.T >= 8) {
-        constexpr int CLI = DG_CLUSTER_I, CLJ = DG_CLUSTER_J;
+        constexpr int CLI = DIGITS == 1 ? DG_CMO_CLUSTER_I : DG_CLUSTER_I, CLJ = DG_CLUSTER_J;
         constexpr int TB = DIGITS == 1 ? 2 : 1;                                      // tiles per CTA and side
         const size_t smem = DGKernelCfg<DIGITS, TB>::SMEM;
         auto kern = drmsd_gram_kernel<DIGITS, CLI, CLJ, TB>;
