@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         for (int it = 0; it < 8 && s_star > 0.0 && sqrt(s_star) >= cutoff; ++it) s_star = nextafter(s_star, 0.0);
         for (int it = 0; it < 8 && sqrt(s_star) < cutoff; ++it) s_star = nextafter(s_star, 1.0e300);
     }
-    const float s_lo = (float)(s_star * (1.0 - 3.0e-6)), s_hi = (float)(s_star * (1.0 + 3.0e-6));
+    const float s_mid = (float)s_star, s_band = (float)(s_star * 3.0e-6);
     // one pass over the K entries, 4 k-steps (128 entries) per trip.  Computing: lane = entry within the k-step, so the
     // warp reads 32 CONSECUTIVE atoms j of a row (stride 3 words: no bank conflict; four entries per lane put the four
     // lane groups on the same banks).  Storing: a 4 x 4 byte transpose within each group of four lanes hands lane
@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
     long long sumsq = 0ll;
     uint32_t ncontact = 0u;
     int ii = 0, jj = 1 + lane;                                   // entry k = 32 kk + lane: pair (ii, jj), ii < jj < L
+    float xa0 = x[0], xa1 = x[1], xa2 = x[2];                    // atom ii, reloaded when the row changes
     const int K32 = valid ? (int)K : 0, ks32 = (int)ks;          // K < 2^16 (L <= 296)
     for (int kk0 = 0; kk0 < ks32; kk0 += 4) {
         uint32_t W0 = 0u, W1 = 0u, W2 = 0u;                      // byte s: this lane's entry of k-step kk0 + s
@@ -174,12 +175,15 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
         for (int s4 = 0; s4 < 4; ++s4) {
             const int k = (kk0 + s4) * 32 + lane;
             if (k < K32) {
-                while (jj >= L) { jj += ii + 2 - L; ++ii; }      // next row(s): entry (ii, L + d) is entry (ii + 1, ii + 2 + d)
+                if (jj >= L) {                                   // next row(s): entry (ii, L + d) is entry (ii + 1, ii + 2 + d)
+                    do { jj += ii + 2 - L; ++ii; } while (jj >= L);
+                    xa0 = x[3 * ii]; xa1 = x[3 * ii + 1]; xa2 = x[3 * ii + 2];
+                }
                 if (DIGITS == 3) {
                     // fp32 is enough here: each coordinate difference carries one rounding, the squared distance three more and
                     // the IEEE square root one, so d is right to ~2^-22 -- about the 24-bit quantisation step itself, random in
                     // sign, and 10^3 times below what the 2e-3 A^2 bar allows (the FP64 version of this loop cost twice the time)
-                    const float fx = x[3 * ii] - x[3 * jj], fy = x[3 * ii + 1] - x[3 * jj + 1], fz = x[3 * ii + 2] - x[3 * jj + 2];
+                    const float fx = xa0 - x[3 * jj], fy = xa1 - x[3 * jj + 1], fz = xa2 - x[3 * jj + 2];
                     const float df = __fsqrt_rn(fmaf(fz, fz, fmaf(fy, fy, fx * fx)));
                     const int I = min(__float2int_rn(df * scale_f), (1 << 23) - 65536);          // keeps |g0| <= 127 whatever the rounding
                     const int g2 = (int)(int8_t)(I & 0xff);
@@ -196,12 +200,10 @@ __global__ void __launch_bounds__(DG_PREP_WARPS * 32) drmsd_prep_kernel(const fl
                     // fp32 screen: each difference carries one rounding (relative 2^-24), so the fp32 squared distance
                     // is within 3e-7 of the FP64 one; outside a 3e-6 band around the threshold the fp32 comparison
                     // decides, inside it (about one entry in 10^5) the FP64 evaluation of eq. 6 does
-                    const float fx = x[3 * ii] - x[3 * jj], fy = x[3 * ii + 1] - x[3 * jj + 1], fz = x[3 * ii + 2] - x[3 * jj + 2];
+                    const float fx = xa0 - x[3 * jj], fy = xa1 - x[3 * jj + 1], fz = xa2 - x[3 * jj + 2];
                     const float s2f = fmaf(fz, fz, fmaf(fy, fy, fx * fx));
-                    uint32_t cbit;
-                    if (s2f < s_lo) cbit = 1u;
-                    else if (s2f > s_hi) cbit = 0u;
-                    else cbit = dist2(ii, jj) < s_star ? 1u : 0u;
+                    uint32_t cbit = s2f < s_mid ? 1u : 0u;
+                    if (!(fabsf(s2f - s_mid) > s_band)) cbit = dist2(ii, jj) < s_star ? 1u : 0u;      // also taken by NaN
                     ncontact += cbit;
                     W0 |= cbit << (8 * s4);
                 }
