@@ -11,16 +11,20 @@
 // six int8 products accumulated EXACTLY in int32 TMEM accumulators (|V| <= 3 K 2^14 < 2^31 needs L <= 296), and
 // |d|^2 is taken from the same integers (exact in 64 bits), so quantisation cancels for similar models.
 //
-// Operand plane (one, shared by both operands): P[tile][k-step][digit][4096 B] -- for 128 consecutive models and 32
-// consecutive entries of K, the int8 digit `digit` as a shared-memory image in tcgen05's canonical K-major no-swizzle
-// core-matrix layout (16 row groups x [2 x 128 B]).  Consecutive k-steps of a tile are contiguous, so the A (or B)
-// operand of a stage of KG k-steps is ONE contiguous run fetched by ONE 1-D bulk copy (the per-copy / per-stage
-// handshake, not the bytes, was what limited an earlier layout with eight 2 KB pieces per k-step).
+// Operand plane (one, shared by both operands).  dRMSD: P[tile128][k-step][digit][4096 B] -- for 128 consecutive models
+// and 32 consecutive entries of K, the int8 digit `digit` as a shared-memory image in tcgen05's canonical K-major
+// no-swizzle core-matrix layout (16 row groups x [2 x 128 B]).  CMO: P[tile256][k-step][half][4096 B], so that the 256
+// models of a tile are ONE N = 256 operand and either half an M = 128 operand.  Consecutive k-steps of a tile are
+// contiguous, so an operand of a stage of KG k-steps is ONE contiguous run fetched by ONE 1-D bulk copy (the per-copy /
+// per-stage handshake, not the bytes, was what limited an earlier layout with eight 2 KB pieces per k-step).
 //
-// Kernel: persistent, one CTA per SM, tile = 128 x 128 models, warp 0 = bulk-copy producer (ring of stages of KG
-// k-steps: A and B, each KG x DIGITS x 4 KB), warp 1 = MMA issuer -- per k-step six N = 128 MMAs, level v (TMEM columns
-// 128 v ...) collecting the digit products A(ga).B(gb)^T with ga + gb = v -- warps 2..17 = epilogue (quadrant x
-// column quarter; results are transposed through shared memory so that the stores run along the packed rows).  2 x 2 thread-block clusters multicast the operands (below).
+// Kernel: persistent, one CTA per SM, warp 0 = bulk-copy producer (ring of stages of KG k-steps), warp 1 = MMA issuer,
+// warps 2..17 = epilogue (TMEM lane quadrant x column quarter; results are transposed through shared memory so that the
+// stores run along the packed rows).  dRMSD: tile = 128 x 128 models, 2 x 2 thread-block clusters whose CTAs each fetch
+// half of their A and B runs and multicast them; per k-step four MMAs -- a0.[b0;b1] -> V0|V1, a1.[b0;b1] -> V1|V2 (N = 256),
+// a0.b2 and a2.b0 -> V2 -- level v (TMEM columns 128 v ...) collecting the digit products A(ga).B(gb)^T with ga + gb = v.
+// CMO: every CTA owns a 256 x 256 block (four 128-column accumulators = all of TMEM), two N = 256 MMAs per k-step, 1 x 2
+// clusters (the row tile's run is shared by multicast, each CTA fetches its own column tile) so that all 148 SMs work.
 #pragma once
 #include "common.cuh"
 #include "prep.cuh"
@@ -42,9 +46,8 @@ template <int DIGITS> struct DGCfg {
     static constexpr int STAGE_BYTES = 2 * OPER_BYTES;
     static constexpr int STAGES = (216 * 1024) / STAGE_BYTES;
 };
-// CMO on the cluster path: every CTA owns a DG_TB x DG_TB block of tiles (all 512 TMEM columns as four 128-column
-// accumulators), so a k-step's 2 DG_TB slabs feed DG_TB^2 MMAs -- with 128 x 128 per CTA the single-digit Gram moved
-// 64 B per SM and clock from L2 and ran at the L2's pace (3.1 ms at C3's shape against 0.7 ms of tensor time)
+// CMO on the cluster path: every CTA owns a 2 x 2 block of 128-model tiles (profiles/r01g_next_rows.md has the history:
+// 3.1 ms -> 1.47 ms at C3's shape against 0.7 ms of tensor time)
 #ifndef DG_CMO_CLUSTER_I
 #define DG_CMO_CLUSTER_I 1                     // CMO cluster rows: 2 (2 x 2, 132 SMs) or 1 (1 x 2, all 148 SMs, 1.5 x the L2 reads)
 #endif
@@ -56,7 +59,7 @@ constexpr int DG_THREADS = (2 + DG_EPI_WARPS) * 32;
 constexpr int DG_PREP_WARPS = 8;
 #ifndef DG_CLUSTER_I
 #define DG_CLUSTER_I 2                         // cluster shape of the Gram kernel: CLI tile rows x CLJ tile columns
-#define DG_CLUSTER_J 2                         // (measured at C3's shape with KG = 2: 2x2 6.73 ms, 1x2 6.97 ms)
+#define DG_CLUSTER_J 2                         // (dRMSD, measured at C3's shape: 2x2 6.67 ms, 1x2 6.76 ms whole call)
 #endif
 
 struct __align__(16) DStat {
