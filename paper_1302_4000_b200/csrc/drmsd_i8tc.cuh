@@ -41,10 +41,9 @@ constexpr int DG_SLAB = 4096;                  // bytes of one (tile, k-step, di
 #define DG_KG3 2                               // dRMSD: k-steps per stage (measured Gram time at C3's shape: 1 -> 7.11 ms, 2 -> 6.73 ms)
 #endif
 template <int DIGITS> struct DGCfg {
-    static constexpr int KG = DIGITS == 3 ? DG_KG3 : 4;                 // k-steps per stage (consecutive k-steps are contiguous)
-    static constexpr int OPER_BYTES = KG * DIGITS * DG_SLAB;            // one operand (A or B tile) of a stage: ONE contiguous run
-    static constexpr int STAGE_BYTES = 2 * OPER_BYTES;
-    static constexpr int STAGES = (216 * 1024) / STAGE_BYTES;
+    // k-steps per stage of the 128 x 128-tile kernels (consecutive k-steps are contiguous); the plane's k-step count is
+    // padded to a multiple of it
+    static constexpr int KG = DIGITS == 3 ? DG_KG3 : 4;
 };
 // CMO on the cluster path: every CTA owns a 2 x 2 block of 128-model tiles (profiles/r01g_next_rows.md has the history:
 // 3.1 ms -> 1.47 ms at C3's shape against 0.7 ms of tensor time)
