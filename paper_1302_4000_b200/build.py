@@ -40,8 +40,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     tmp = LIB + f".tmp{os.getpid()}"
-    extra = os.environ.get("CLUSCO_NVCC_EXTRA", "").split()          # e.g. -DI8_EXPERIMENT=1 (developer switches)
-    cmd = [NVCC] + FLAGS + extra + ["-o", tmp] + sources() + ["-lcudart"]
+    cmd = [NVCC] + FLAGS + ["-o", tmp] + sources() + ["-lcudart"]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose or r.returncode != 0:
         sys.stderr.write(r.stdout + r.stderr)

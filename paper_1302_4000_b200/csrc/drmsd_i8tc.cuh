@@ -37,9 +37,7 @@ constexpr int DG_MAX_L = 296;                  // 3 K 2^14 < 2^31 with K = L(L-1
 constexpr int DG_TILE = 128;
 constexpr int DG_SLAB = 4096;                  // bytes of one (tile, k-step, digit) image: 128 rows x 32 entries
 // DIGITS = 3: dRMSD (24-bit fixed-point distances); DIGITS = 1: CMO (0/1 contact maps, eq. 6-7) on the same kernels
-#ifndef DG_KG3
-#define DG_KG3 2                               // dRMSD: k-steps per stage (measured Gram time at C3's shape: 1 -> 7.11 ms, 2 -> 6.73 ms)
-#endif
+constexpr int DG_KG3 = 2;                      // dRMSD: k-steps per stage (measured Gram time at C3's shape: 1 -> 7.11 ms, 2 -> 6.73 ms)
 template <int DIGITS> struct DGCfg {
     // k-steps per stage of the 128 x 128-tile kernels (consecutive k-steps are contiguous); the plane's k-step count is
     // padded to a multiple of it
@@ -47,19 +45,13 @@ template <int DIGITS> struct DGCfg {
 };
 // CMO on the cluster path: every CTA owns a 2 x 2 block of 128-model tiles (profiles/r01g_next_rows.md has the history:
 // 3.1 ms -> 1.47 ms at C3's shape against 0.7 ms of tensor time)
-#ifndef DG_CMO_CLUSTER_I
-#define DG_CMO_CLUSTER_I 1                     // CMO cluster rows: 2 (2 x 2, 132 SMs) or 1 (1 x 2, all 148 SMs, 1.5 x the L2 reads)
-#endif
-#ifndef DG_KG1B
-#define DG_KG1B 2                              // CMO, blocked: k-steps per stage (measured: 2 -> 1.69 ms, 4 -> 1.71 ms whole call)
-#endif
+constexpr int DG_CMO_CLUSTER_I = 1;            // CMO cluster rows: 2 (2 x 2, 132 SMs) or 1 (1 x 2, all 148 SMs, 1.5 x the L2 reads)
+constexpr int DG_KG1B = 2;                     // CMO, blocked: k-steps per stage (measured: 2 -> 1.69 ms, 4 -> 1.71 ms whole call)
 constexpr int DG_EPI_WARPS = 16;               // 4 TMEM lane quadrants x 4 column quarters of a tile
 constexpr int DG_THREADS = (2 + DG_EPI_WARPS) * 32;
 constexpr int DG_PREP_WARPS = 8;
-#ifndef DG_CLUSTER_I
-#define DG_CLUSTER_I 2                         // cluster shape of the Gram kernel: CLI tile rows x CLJ tile columns
-#define DG_CLUSTER_J 2                         // (dRMSD, measured at C3's shape: 2x2 6.67 ms, 1x2 6.76 ms whole call)
-#endif
+constexpr int DG_CLUSTER_I = 2;                // cluster shape of the Gram kernel: CLI tile rows x CLJ tile columns
+constexpr int DG_CLUSTER_J = 2;                // (dRMSD, measured at C3's shape: 2x2 6.67 ms, 1x2 6.76 ms whole call)
 
 struct __align__(16) DStat {
     double T;          // KAPPA^2 sum_k d_k^2 of the quantised distances, true scale (Angstrom^2); NaN poisons the model
@@ -454,9 +446,6 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
                     constexpr uint32_t SL = DG_SLAB >> 4;
 #pragma unroll
                     for (int q = 0; q < KG; ++q) {
-#if defined(DG_EXPERIMENT) && (DG_EXPERIMENT & 2)                  // developer switch: operand delivery only (one MMA per tile)
-                        if (kg > 0 || q > 0) continue;
-#endif
                         const uint32_t acc = (kg > 0 || q > 0) ? 1u : 0u;
                         const uint32_t aq = a_lo + q * DIGITS * SL, bq = b_lo + q * DIGITS * SL;
                         if (TB > 1) {
@@ -506,11 +495,7 @@ __global__ void __launch_bounds__(DG_THREADS, 1) drmsd_gram_kernel(const DGParam
 #pragma unroll 1
             for (int sub = 0; sub < TB * TB; ++sub) {            // the tiles of this CTA's block
                 const int32_t I = TB * (CLI * SI + ri) + sub / TB, J = TB * (CLJ * SJ + rj) + sub % TB;
-#if defined(DG_EXPERIMENT) && (DG_EXPERIMENT & 1)                  // developer switch: no epilogue work
-                const bool active = false;
-#else
                 const bool active = I < P.T && J < P.T && I <= J;    // a cluster's block may hang over the edge / the diagonal
-#endif
                 const int64_t ibase = (int64_t)min(I, P.T - 1) * DG_TILE + quad * 32;
                 const int64_t i = ibase + lane;
                 const DStat si = P.stat[i];                          // slots beyond N hold neutral records

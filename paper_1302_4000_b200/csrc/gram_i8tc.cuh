@@ -333,13 +333,9 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
 #pragma unroll
                 for (int k = 0; k < KS; ++k) {
                     const uint64_t db = DESC_HI | (b_lo + k * (I8_B_SLAB >> 4));
-#if defined(I8_EXPERIMENT) && I8_EXPERIMENT == 2          // developer switch: one MMA per tile (epilogue-side time only)
-                    if (k == 0) ptx::mma_i8_ts(d, a_tm, db, ID144, 0);
-#else
                     ptx::mma_i8_ts(d, a_tm + 8 * k, db, ID144, k > 0);
                     ptx::mma_i8_ts(d + 48, a_tm + 8 * (KS + k), db, ID96, 1);
                     ptx::mma_i8_ts(d + 96, a_tm + 8 * (2 * KS + k), db, ID48, 1);
-#endif
                 }
                 ptx::tc_commit(B_EMPTY(stage));
                 ptx::tc_commit(ACC_FULL(buf));
@@ -411,13 +407,9 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             }
         };
         auto finish_pending = [&](const Pending& pend) {
-#if defined(I8_EXPERIMENT) && (I8_EXPERIMENT == 1 || I8_EXPERIMENT >= 3)   // developer switch: no eq. 2 arithmetic
-            const float2 c = make_float2(pend.inv.c2.x + pend.inv.c1.x + pend.Thi, pend.inv.c2.y + pend.inv.d.y + pend.Thj.y);
-#else
             const float2 c = eq2_finish(eq2_energy(pend.inv), make_float2(pend.Thi, pend.Thi),
                                         make_float2(pend.Tlo, pend.Tlo), make_float2(pend.pw, pend.pw), pend.Thj,
                                         pend.Tlj, pend.pwj, P.invLk);
-#endif
             if (MODE == SINK_STORE) {
                 if (pend.ok0) pend.dst[0] = c.x;
                 if (pend.ok1) pend.dst[4] = c.y;
@@ -494,11 +486,6 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             // m[3p+q] = (.x, .y): pairs (row model r, column model c4 + 8 half) and (.., + 4); Gram sums in units
             // of 2^46.  The two pairs of a thread go through the closed form together, on packed fp32 arithmetic.
             float2 m[9];
-#if defined(I8_EXPERIMENT) && I8_EXPERIMENT >= 3              // developer switch: no TMEM loads, no arithmetic
-#pragma unroll
-            for (int q = 0; q < 9; ++q) m[q] = make_float2((float)(n + q), (float)(n + q + 1));
-            if (have_prev) finish_pending(prev);
-#else
             {
                 // levels 1 and 2 first: T = 2^8 V1 + V2 fits int32 (|T| < 2^31 for L <= 256 because |d0| <= 127)
                 uint32_t v1[3][2][4], v2[3][2][4];
@@ -537,17 +524,12 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                     m[6 + q] = __ffma2_rn(make_float2(F(1, 0), F(1, 1)), s14, m[6 + q]);
                 }
             }
-#endif
             // the accumulator buffer is free again
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
 
-#if defined(I8_EXPERIMENT) && (I8_EXPERIMENT == 1 || I8_EXPERIMENT >= 3)   // developer switch: no eq. 2 arithmetic
-            pend.inv.c2 = m[0]; pend.inv.c1 = m[4]; pend.inv.d = m[8];
-#else
             pend.inv = eq2_invariants(m);
-#endif
             pend.Thi = si.Thi; pend.Tlo = si.Tlo; pend.pw = si.pw;
             pend.Thj = make_float2(sj0.Thi, sj1.Thi);
             pend.Tlj = make_float2(sj0.Tlo, sj1.Tlo);

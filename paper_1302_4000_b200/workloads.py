@@ -39,6 +39,7 @@ class Ensemble:
     mirror_idx: np.ndarray = field(default_factory=lambda: np.zeros(0, np.int64))
     rigid_copy_idx: np.ndarray = field(default_factory=lambda: np.zeros(0, np.int64))
     cluster_id: np.ndarray | None = None    # (N,) for C3
+    stats: dict | None = None               # shape record of the native (chain_shape), logged beside every result
 
     @property
     def N(self) -> int:
@@ -81,6 +82,29 @@ def random_walk_chain(L: int, rng: np.random.Generator) -> np.ndarray:
     return x
 
 
+def chain_shape(x: np.ndarray) -> dict:
+    """Shape record of one chain, logged for every config (generator step 1): the native's
+    R_g^2 varies ~8x over seeds and every fp32 error term of the GPU path scales with it, so a result without this
+    record cannot be placed.  Plain FP64 numpy on the un-noised chain; neither the oracle nor the CUDA path uses it."""
+    a = np.asarray(x, np.float64)
+    a = a - a.mean(0)
+    ev = np.linalg.eigvalsh(a.T @ a / a.shape[0])[::-1]
+    return {"rg2": float(ev.sum()), "gyration_eigenvalues": [float(v) for v in ev],
+            "max_abs_centred": float(np.abs(a).max())}
+
+
+# The generator's tail: for each chain length the seed s in 0..199 whose random_walk_chain(L, default_rng(s)) has the
+# LARGEST R_g^2 (most extended chain; tests/test_workloads.py re-derives the table).  The GPU path's error grows with
+# R_g^2, so parity is also asked on ensembles built on these natives, not only on the five configs' own natives
+# (R_g^2 479..969 A^2, below the generator's median at their lengths).
+TAIL_SEEDS = {100: 63, 140: 47, 150: 69, 215: 38, 250: 48}
+
+
+def tail_native(L: int) -> np.ndarray:
+    """The most extended of the 200 chains random_walk_chain(L, default_rng(0..199))  (R_g^2 = 4289 A^2 at L = 250)."""
+    return random_walk_chain(L, np.random.default_rng(TAIL_SEEDS[L]))
+
+
 def random_rotations(n: int, rng: np.random.Generator) -> np.ndarray:
     """n proper rotations, uniform on SO(3), from normalised 4-vectors of standard normals."""
     q = rng.normal(size=(n, 4))
@@ -114,10 +138,12 @@ def _noisy_decoys(native, n, lo, hi, rng_noise):
 
 
 def make_decoys(config_index: int, N: int, L: int, sigma_lo: float, sigma_hi: float,
-                n_mirror: int = 0, n_rigid: int = 0, name: str | None = None) -> Ensemble:
-    """Configs C1, C2, C4: native + iid Gaussian noise, optional mirrors / rigid copies, rigid transform."""
+                n_mirror: int = 0, n_rigid: int = 0, name: str | None = None,
+                native: np.ndarray | None = None) -> Ensemble:
+    """Configs C1, C2, C4: native + iid Gaussian noise, optional mirrors / rigid copies, rigid transform.
+    `native` (L, 3) replaces the config's own seeded chain (the tail ensembles)."""
     r_native, r_noise, r_rigid, r_struct = _streams(config_index)
-    native = random_walk_chain(L, r_native)
+    native = random_walk_chain(L, r_native) if native is None else np.asarray(native, np.float64)
     y, sigma = _noisy_decoys(native, N, sigma_lo, sigma_hi, r_noise)
     # specials (SURVEY.md Q12): first n_mirror decoys are mirrored (x -> -x) BEFORE the rigid
     # transform, the next n_rigid are the native itself (sigma = 0); then a seeded shuffle.
@@ -133,14 +159,15 @@ def make_decoys(config_index: int, N: int, L: int, sigma_lo: float, sigma_hi: fl
     z = rigid_transform(y, r_rigid)
     nat = rigid_transform(native[None], r_rigid)[0]
     return Ensemble(name or f"C{config_index}", z.astype(np.float32), nat.astype(np.float32), sigma,
-                    np.sort(inv[mirror]), np.sort(inv[rigid]))
+                    np.sort(inv[mirror]), np.sort(inv[rigid]), stats=chain_shape(native))
 
 
 def make_clusters(config_index: int, N: int, L: int, n_clusters: int = 20, centre_sigma: float = 4.0,
-                  sigma_lo: float = 0.3, sigma_hi: float = 2.0, name: str | None = None) -> Ensemble:
+                  sigma_lo: float = 0.3, sigma_hi: float = 2.0, name: str | None = None,
+                  native: np.ndarray | None = None) -> Ensemble:
     """Config C3: n_clusters cluster centres = native + N(0, centre_sigma^2); members around them."""
     r_native, r_noise, r_rigid, r_struct = _streams(config_index)
-    native = random_walk_chain(L, r_native)
+    native = random_walk_chain(L, r_native) if native is None else np.asarray(native, np.float64)
     centres = native[None] + r_noise.normal(size=(n_clusters, L, 3)) * centre_sigma
     cid = np.arange(N) % n_clusters
     sigma = r_noise.uniform(sigma_lo, sigma_hi, size=N)
@@ -150,11 +177,12 @@ def make_clusters(config_index: int, N: int, L: int, n_clusters: int = 20, centr
     z = rigid_transform(y, r_rigid)
     nat = rigid_transform(native[None], r_rigid)[0]
     return Ensemble(name or f"C{config_index}", z.astype(np.float32), nat.astype(np.float32), sigma,
-                    cluster_id=cid)
+                    cluster_id=cid, stats=chain_shape(native))
 
 
 def make_one_vs_all(config_index: int, N: int, L: int, sigma_lo: float = 0.5, sigma_hi: float = 10.0,
-                    chunk: int = 100_000, chunks: range | None = None, name: str | None = None) -> Ensemble:
+                    chunk: int = 100_000, chunks: range | None = None, name: str | None = None,
+                    native: np.ndarray | None = None) -> Ensemble:
     """Config C5: one native vs N decoys, generated in independently seeded chunks of `chunk` models.
 
     `chunks` selects which chunks to produce (default: all), so a test can regenerate any slice
@@ -162,7 +190,8 @@ def make_one_vs_all(config_index: int, N: int, L: int, sigma_lo: float = 0.5, si
     """
     ss = np.random.SeedSequence(SEED_BASE + config_index)
     s_native, s_rigid_native, s_chunks = ss.spawn(3)
-    native = random_walk_chain(L, np.random.Generator(np.random.PCG64(s_native)))
+    native = (random_walk_chain(L, np.random.Generator(np.random.PCG64(s_native))) if native is None
+              else np.asarray(native, np.float64))
     nat = rigid_transform(native[None], np.random.Generator(np.random.PCG64(s_rigid_native)))[0]
     n_chunks = (N + chunk - 1) // chunk
     chunk_seeds = s_chunks.spawn(n_chunks)
@@ -176,7 +205,7 @@ def make_one_vs_all(config_index: int, N: int, L: int, sigma_lo: float = 0.5, si
         sig.append(sigma)
     coords = np.concatenate(out) if out else np.zeros((0, L, 3), np.float32)
     return Ensemble(name or f"C{config_index}", coords, nat.astype(np.float32),
-                    np.concatenate(sig) if sig else np.zeros(0))
+                    np.concatenate(sig) if sig else np.zeros(0), stats=chain_shape(native))
 
 
 # ---- BASELINE.json's five configurations -------------------------------------------------------
@@ -201,6 +230,22 @@ def make_config(name: str, N: int | None = None, **kw) -> Ensemble:
     if c["kind"] == "clusters":
         return make_clusters(k, n, c["L"], name=name)
     return make_one_vs_all(k, n, c["L"], *c["sigma"], name=name, **kw)
+
+
+def make_tail(shape: str, N: int, L: int | None = None) -> Ensemble:
+    """An ensemble with the noise recipe of config `shape` ("C2".."C5") built on the generator's most extended
+    native of length L (default: the config's own L; TAIL_SEEDS).  Streams: those of config index 100 + k, so the
+    tail ensembles share no random numbers with C1..C5."""
+    c = CONFIGS[shape]
+    k = int(shape[1:])
+    L = c["L"] if L is None else L
+    nat = tail_native(L)
+    name = f"{shape}-tail(L={L})"
+    if c["kind"] == "decoys":
+        return make_decoys(100 + k, N, L, *c["sigma"], name=name, native=nat)
+    if c["kind"] == "clusters":
+        return make_clusters(100 + k, N, L, name=name, native=nat)
+    return make_one_vs_all(100 + k, N, L, *c["sigma"], chunk=max(1, N), name=name, native=nat)
 
 
 def packed_index(i, j, N):

@@ -72,12 +72,35 @@ def test_cmo_full_size_sampled(clusco):
     ens = wl.make_config("C3")
     got = clusco.clusco_cmo_allpairs(_dev(ens.coords), 8.0).cpu().numpy()
     rng = np.random.default_rng(11)
-    pi = rng.integers(0, ens.N - 1, 400)
+    pi = rng.integers(0, ens.N - 1, 20_000)
     pj = np.array([rng.integers(i + 1, ens.N) for i in pi])
     pi = np.concatenate([pi, [0, 0, ens.N - 2, 127, 128]])
     pj = np.concatenate([pj, [1, ens.N - 1, ens.N - 1, 128, 9999]])
     want = oracle.cmo_pairs(ens.coords, 8.0, pi, pj).astype(np.float32)
     assert np.array_equal(got[wl.packed_index(pi, pj, ens.N)], want)
+
+
+def test_cmo_cluster_path_large_K_every_pair(clusco):
+    """The cluster kernel (N >= 897) with a long contraction: L = 160, K = 12 720 contact bits per model."""
+    ens = wl.make_tail("C2", 900, 140)
+    x = np.concatenate([ens.coords, ens.coords[:, :20]], axis=1).copy()
+    want = oracle.cmo_allpairs(x, 8.0).astype(np.float32)
+    got = clusco.clusco_cmo_allpairs(_dev(x), 8.0).cpu().numpy()
+    assert np.array_equal(got, want)
+
+
+def test_cmo_cluster_path_max_L_sampled(clusco):
+    """L = 296 (K = 43 660, the largest supported), cluster path, sampled pairs."""
+    rng = np.random.default_rng(297)
+    N, L = 1000, 296
+    nat = wl.random_walk_chain(L, rng)
+    y = nat[None] + rng.normal(size=(N, L, 3)) * rng.uniform(0.0, 3.0, size=(N, 1, 1))
+    x = wl.rigid_transform(y, rng).astype(np.float32)
+    got = clusco.clusco_cmo_allpairs(_dev(x), 8.0).cpu().numpy()
+    pi = rng.integers(0, N - 1, 15_000)
+    pj = np.array([rng.integers(i + 1, N) for i in pi])
+    want = oracle.cmo_pairs(x, 8.0, pi, pj).astype(np.float32)
+    assert np.array_equal(got[wl.packed_index(pi, pj, N)], want)
 
 
 @pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12), (2049, 20)])

@@ -92,12 +92,48 @@ def test_drmsd_full_size_sampled(clusco):
     ens = wl.make_config("C3")
     got = clusco.clusco_drmsd_allpairs(_dev(ens.coords)).cpu().numpy()
     rng = np.random.default_rng(7)
-    pi = rng.integers(0, ens.N - 1, 400)
+    pi = rng.integers(0, ens.N - 1, 20_000)
     pj = np.array([rng.integers(i + 1, ens.N) for i in pi])
     pi = np.concatenate([pi, [0, 0, ens.N - 2, 127, 128]])
     pj = np.concatenate([pj, [1, ens.N - 1, ens.N - 1, 128, 9999]])
     d_ref, d2_ref = oracle.drmsd_pairs(ens.coords, pi, pj)
     _check(got[wl.packed_index(pi, pj, ens.N)], d_ref, d2_ref, "C3 sampled")
+
+
+def test_drmsd_tail_every_pair(clusco):
+    """C3's recipe on the generator's most extended native (R_g^2 = 4289 A^2, the largest distances and sums)."""
+    ens = wl.make_tail("C3", 400)
+    d_ref, d2_ref = oracle.drmsd_allpairs(ens.coords)
+    got = clusco.clusco_drmsd_allpairs(_dev(ens.coords)).cpu().numpy()
+    _check(got, d_ref, d2_ref, ens.name)
+    print(f"{ens.name}: max|dd2| = {np.abs(got.astype(np.float64) ** 2 - d2_ref).max():.2e}")
+
+
+def test_drmsd_cluster_path_large_K_every_pair(clusco):
+    """The 2 x 2 cluster kernel (N >= 897) with a long contraction: L = 160, K = 12 720 (398 k-steps, ragged last one)."""
+    ens = wl.make_tail("C2", 900, 140)
+    x = np.concatenate([ens.coords, ens.coords[:, :20]], axis=1).copy()        # L = 160: the chain plus a repeated piece
+    d_ref, d2_ref = oracle.drmsd_allpairs(x)
+    got = clusco.clusco_drmsd_allpairs(_dev(x)).cpu().numpy()
+    _check(got, d_ref, d2_ref, "cluster path L=160")
+
+
+def test_drmsd_cluster_path_max_L_sampled(clusco):
+    """L = 296 is the int32 bound of the level sums (3 K 2^14 < 2^31): cluster path, sampled pairs, extended chains."""
+    rng = np.random.default_rng(296)
+    N, L = 1000, 296
+    nat = wl.random_walk_chain(L, rng)
+    y = nat[None] + rng.normal(size=(N, L, 3)) * rng.uniform(0.0, 3.0, size=(N, 1, 1))
+    x = wl.rigid_transform(y, rng).astype(np.float32)
+    x[1] = x[0]
+    got = clusco.clusco_drmsd_allpairs(_dev(x)).cpu().numpy()
+    pi = rng.integers(0, N - 1, 15_000)
+    pj = np.array([rng.integers(i + 1, N) for i in pi])
+    pi = np.concatenate([pi, [0, 0, N - 2, 127, 128]])
+    pj = np.concatenate([pj, [1, N - 1, N - 1, 128, 999]])
+    d_ref, d2_ref = oracle.drmsd_pairs(x, pi, pj)
+    _check(got[wl.packed_index(pi, pj, N)], d_ref, d2_ref, "max L sampled")
+    assert got[0] == 0.0
 
 
 @pytest.mark.parametrize("N,L", [(1100, 30), (1024, 12), (2049, 20)])

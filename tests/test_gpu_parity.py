@@ -85,34 +85,93 @@ def test_allpairs_C1_specials(clusco, c1):
         assert out[wl.packed_index(i, j, c1.N)] > 1.0
 
 
-# ---- full-size configs in the launch configuration bench.py times: sampled outputs --------------------
+# ---- full-size configs in the launch configuration bench.py times ------------------------------------------
 
-@pytest.mark.parametrize("cfg", ["C3", "C4"])
-def test_allpairs_full_size_sampled(clusco, cfg):
-    ens = wl.make_config(cfg)
+def test_allpairs_C3_full_size_every_pair(clusco):
+    """C3 as bench.py times it (10 000 x 250, 49 995 000 pairs): EVERY pair against the oracle, in row blocks."""
+    import torch
+    ens = wl.make_config("C3")
+    N = ens.N
+    out = clusco.clusco_crmsd_allpairs(_dev(ens.coords))
+    assert out.numel() == N * (N - 1) // 2 and bool(torch.isfinite(out).all())
+    got = out.cpu().numpy()
+    worst = 0.0
+    bounds = list(range(0, N, 1000)) + [N]
+    for lo, hi in zip(bounds, bounds[1:]):
+        c_ref, c2_ref = oracle.crmsd_rows(ens.coords, lo, hi)
+        k0, k1 = lo * (2 * N - lo - 1) // 2, hi * (2 * N - hi - 1) // 2
+        worst = max(worst, assert_parity(got[k0:k1], c_ref, c2_ref, f"C3 full size rows {lo}..{hi}"))
+    print(f"C3 full size, every pair ({got.size}): max|dc2| = {worst:.2e}  (native R_g^2 = {ens.stats['rg2']:.0f} A^2)")
+
+
+def test_allpairs_C4_full_size_sampled(clusco):
+    """C4 as bench.py times it (30 000 x 100, 4.5e8 pairs): 1e7 random pairs and whole rows (first / last /
+    tile-boundary rows) against the oracle; finiteness and the bound c^2 <= R_A^2 + R_B^2 on every pair."""
+    import torch
+    ens = wl.make_config("C4")
     N = ens.N
     rng = np.random.default_rng(99)
     out = clusco.clusco_crmsd_allpairs(_dev(ens.coords))
     assert out.numel() == N * (N - 1) // 2
-    # (i) random pairs, (ii) whole rows incl. first / last / tile-boundary rows
-    pi = rng.integers(0, N, 200_000)
-    pj = rng.integers(0, N, 200_000)
+    pi = rng.integers(0, N, 10_000_000)
+    pj = rng.integers(0, N, 10_000_000)
     keep = pi != pj
     pi, pj = np.minimum(pi, pj)[keep], np.maximum(pi, pj)[keep]
-    rows = [0, 1, 127, 128, 129, N // 2, N - 130, N - 2] + list(rng.integers(0, N - 1, 8))
+    rows = [0, 1, 31, 32, 127, 128, 129, N // 2, N - 130, N - 33, N - 2] + list(rng.integers(0, N - 1, 8))
     for r in rows:
         pi = np.concatenate([pi, np.full(N - 1 - r, r)])
         pj = np.concatenate([pj, np.arange(r + 1, N)])
     c_ref, c2_ref = oracle.crmsd_pairs(ens.coords, pi, pj)
-    import torch
     idx = torch.from_numpy(wl.packed_index(pi, pj, N)).cuda()
     got = out[idx].cpu().numpy()
-    worst = assert_parity(got, c_ref, c2_ref, f"{cfg} full size")
-    print(f"{cfg} full size, {len(pi)} sampled pairs: max|dc2| = {worst:.2e}")
-    # properties that hold at any size: finite, within the bounds (R_A-R_B)^2 <= c^2 <= R_A^2+R_B^2
+    worst = assert_parity(got, c_ref, c2_ref, "C4 full size")
+    print(f"C4 full size, {len(pi)} sampled pairs: max|dc2| = {worst:.2e}")
     assert bool(torch.isfinite(out).all())
     _, r2 = oracle.center(ens.coords)
     assert float(out.max()) ** 2 <= 2 * r2.max() + 1e-2
+
+
+# ---- the generator's tail: the same noise recipes on the most extended native of 200 seeds --------------------
+# Every fp32 error term of the path scales with R_g^2 (SURVEY.md 8(c) error budget); the five configs' own natives
+# have R_g^2 = 479..969 A^2, the generator reaches 4289 A^2 at L = 250 (workloads.TAIL_SEEDS).
+
+@pytest.mark.parametrize("shape,N,L", [("C3", 3000, None), ("C4", 3000, None), ("C2", 2000, 140), ("C3", 2000, 215),
+                                       ("C2", 1500, 250)])
+def test_allpairs_tail_every_pair(clusco, shape, N, L):
+    ens = wl.make_tail(shape, N, L)
+    c_ref, c2_ref = oracle.crmsd_allpairs(ens.coords)
+    for eng in _engines(clusco, ens.L):
+        out = clusco.clusco_crmsd_allpairs(_dev(ens.coords), engine=eng).cpu().numpy()
+        worst = assert_parity(out, c_ref, c2_ref, f"{ens.name} engine {eng}")
+        print(f"{ens.name} N={ens.N} R_g^2={ens.stats['rg2']:.0f}: engine={eng} max|dc2| = {worst:.2e} "
+              f"(bar 2e-3), max|dc|(c>=0.5) = {np.abs(out - c_ref)[c_ref >= 0.5].max():.2e} (bar 1e-3)")
+
+
+def test_one_vs_all_tail(clusco):
+    ens = wl.make_tail("C5", 50_000)
+    c_ref, c2_ref = oracle.crmsd_one_vs_all(ens.native, ens.coords)
+    out = clusco.clusco_crmsd_one_vs_all(_dev(ens.native), _dev(ens.coords)).cpu().numpy()
+    worst = assert_parity(out, c_ref, c2_ref, ens.name)
+    print(f"{ens.name} R_g^2={ens.stats['rg2']:.0f}: max|dc2| = {worst:.2e}")
+
+
+# ---- every tensor-core instantiation: KS = ceil(L / 32) = 1..8 ------------------------------------------------
+# L = 129..224 (KS = 5, 6, 7) have their own B-ring depth and TMEM footprint of the A operand; the paper's own
+# benchmark proteins of 140 and 215 residues (PAPER.md:140, 229) fall there.  N is chosen so that the 148 CTAs each
+# walk several row tiles (ragged N: partial last row and column tiles).
+
+@pytest.mark.parametrize("N,L", [(1100, 129), (1500, 140), (1201, 160), (1333, 192), (1500, 215), (1111, 224),
+                                 (1290, 32), (1177, 64), (1403, 96), (1100, 256)])
+def test_allpairs_every_kstep_count(clusco, N, L):
+    rng = np.random.default_rng(31 * N + L)
+    nat = wl.tail_native(L) if L in wl.TAIL_SEEDS else wl.random_walk_chain(L, rng)
+    y = nat[None] + rng.normal(size=(N, L, 3)) * rng.uniform(0.2, 5.0, size=(N, 1, 1))
+    x = wl.rigid_transform(y, rng).astype(np.float32)
+    c_ref, c2_ref = oracle.crmsd_allpairs(x)
+    for eng in _engines(clusco, L):
+        out = clusco.clusco_crmsd_allpairs(_dev(x), engine=eng).cpu().numpy()
+        worst = assert_parity(out, c_ref, c2_ref, f"N={N} L={L} engine {eng}")
+        print(f"N={N} L={L} KS={(L + 31) // 32} engine={eng}: max|dc2| = {worst:.2e}")
 
 
 # ---- ragged shapes, tile edges, degenerate inputs -----------------------------------------------------
@@ -251,16 +310,39 @@ def test_one_vs_all_full_size_sampled(clusco):
 DELTA = 1.5e-3
 
 
-def _consumer_cases():
+def _ks_case(N, L, seed):
+    rng = np.random.default_rng(seed)
+    nat = wl.tail_native(L) if L in wl.TAIL_SEEDS else wl.random_walk_chain(L, rng)
+    y = nat[None] + rng.normal(size=(N, L, 3)) * rng.uniform(0.2, 4.0, size=(N, 1, 1))
+    return wl.rigid_transform(y, rng).astype(np.float32)
+
+
+def _long_chain():
     rng = np.random.default_rng(99)
-    long_chain = (rng.normal(size=(150, 300, 3)) * 8 + rng.uniform(-40, 40, size=(150, 1, 3))).astype(np.float32)
-    return [("C1", wl.make_config("C1").coords, 3.2), ("C2[:1000]", wl.make_config("C2", N=1000).coords, 6.0),
-            ("C3[:700]", wl.make_config("C3", N=700).coords, 3.2), ("L300-ffma", long_chain, 18.5)]
+    return (rng.normal(size=(150, 300, 3)) * 8 + rng.uniform(-40, 40, size=(150, 1, 3))).astype(np.float32)
 
 
-@pytest.mark.parametrize("case", range(4))
+# (name, coordinates, cut-off); cases 4..7: KS = 5, 6, 7 instantiations and the tail native (R_g^2 4289)
+_CONSUMER_CASES = [
+    ("C1", lambda: wl.make_config("C1").coords, 3.2),
+    ("C2[:1000]", lambda: wl.make_config("C2", N=1000).coords, 6.0),
+    ("C3[:700]", lambda: wl.make_config("C3", N=700).coords, 3.2),
+    ("L300-ffma", _long_chain, 18.5),
+    ("KS5 L=140", lambda: _ks_case(1300, 140, 5), 4.0),
+    ("KS6 L=192", lambda: _ks_case(1209, 192, 6), 4.0),
+    ("KS7 L=215", lambda: _ks_case(1500, 215, 7), 4.0),
+    ("C3-tail[:1500]", lambda: wl.make_tail("C3", 1500).coords, 3.2),
+]
+
+
+def _consumer_case(k):
+    name, make, cutoff = _CONSUMER_CASES[k]
+    return name, make(), cutoff
+
+
+@pytest.mark.parametrize("case", range(len(_CONSUMER_CASES)))
 def test_pairs_below_matches_oracle(clusco, case):
-    name, x, cutoff = _consumer_cases()[case]
+    name, x, cutoff = _consumer_case(case)
     N = x.shape[0]
     c_ref, c2_ref = oracle.crmsd_allpairs(x)
     must = set(np.nonzero(c_ref < cutoff - DELTA)[0].tolist())
@@ -289,9 +371,9 @@ def test_pairs_below_matches_oracle(clusco, case):
     assert int(count3.item()) == n
 
 
-@pytest.mark.parametrize("case", range(4))
+@pytest.mark.parametrize("case", range(len(_CONSUMER_CASES)))
 def test_rowstats_match_oracle(clusco, case):
-    name, x, cutoff = _consumer_cases()[case]
+    name, x, cutoff = _consumer_case(case)
     N = x.shape[0]
     rs_ref, _ = oracle.rowstats(x, cutoff)
     _, lo = oracle.rowstats(x, cutoff - DELTA)

@@ -56,3 +56,26 @@ def test_packed_index_is_row_major_triu():
     N = 7
     iu = np.triu_indices(N, 1)
     assert np.array_equal(wl.packed_index(iu[0], iu[1], N), np.arange(N * (N - 1) // 2))
+
+
+def test_tail_seeds_are_the_most_extended_of_200():
+    """workloads.TAIL_SEEDS names, per chain length, the seed in 0..199 with the largest R_g^2 (the
+    native's R_g^2 varies ~8x over seeds and the GPU path's error scales with it)."""
+    for L, seed in wl.TAIL_SEEDS.items():
+        rg2 = [wl.chain_shape(wl.random_walk_chain(L, np.random.default_rng(s)))["rg2"] for s in range(200)]
+        assert int(np.argmax(rg2)) == seed, (L, int(np.argmax(rg2)))
+    assert abs(wl.chain_shape(wl.tail_native(250))["rg2"] - 4288.75) < 0.01
+    assert wl.chain_shape(wl.random_walk_chain(250, np.random.default_rng(0)))["rg2"] < np.median(rg2) * 4
+
+
+def test_chain_shape_record_and_tail_ensembles():
+    x = np.array([[0.0, 0, 0], [2.0, 0, 0], [0, 4.0, 0], [2.0, 4.0, 0]])           # 2 x 4 rectangle
+    st = wl.chain_shape(x)
+    assert np.allclose(st["gyration_eigenvalues"], [4.0, 1.0, 0.0]) and abs(st["rg2"] - 5.0) < 1e-12
+    assert st["max_abs_centred"] == 2.0
+    e = wl.make_tail("C3", 40)
+    assert e.coords.shape == (40, 250, 3) and abs(e.stats["rg2"] - 4288.75) < 0.01
+    assert not np.array_equal(e.coords[:40], wl.make_config("C3", N=40).coords)
+    e5 = wl.make_tail("C5", 30)
+    assert e5.coords.shape == (30, 150, 3) and e5.native.shape == (150, 3)
+    assert wl.make_config("C3", N=40).stats["rg2"] < 1000.0
