@@ -177,21 +177,56 @@ __device__ __forceinline__ EPairT<V> eq2_energy(const V m[9])
     return eq2_energy(eq2_invariants(m));
 }
 
-// The last line of eq. 2 for a pair (i, j) whose models carry power-of-two scales 2^ei, 2^ej:
-//   m[] holds the Gram sums of the SCALED coordinates, (Shi,Slo) the two-float sums of squares of the
-//   scaled coordinates, so   L c^2 2^-(ei+ej) = S_i 2^(ei-ej) + S_j 2^(ej-ei) - 2 E   with every scaling exact.
-__device__ __forceinline__ float eq2_crmsd(const float m[9], float Shi_i, float Slo_i, int ei,
-                                           float Shi_j, float Slo_j, int ej, float invL)
+// ---- FP64 form of the closed form for a pair (i, j) whose models carry power-of-two scales 2^ei, 2^ej:  m[] holds the
+// Gram sums of the SCALED coordinates, S the sums of squares of the scaled coordinates, so
+//   L c^2 2^-(ei+ej) = S_i 2^(ei-ej) + S_j 2^(ej-ei) - 2 E   with every scaling exact.   (The CUDA-core engine, which serves the long chains whose R_g^2 -- and with it
+// every fp32 error term of the form above -- is largest).  Same mathematics: invariants of M, Viete's largest root and
+// the deflated start value in fp32 (only a starting value), then Newton steps on the quartic in FP64 and the last
+// line of eq. 2 in FP64, so that the result carries the rounding of the Gram sums and nothing else.
+__device__ __forceinline__ float eq2_crmsd_f64(const double m[9], double S_i, int ei, double S_j, int ej, double invL)
 {
-    const EPair e = eq2_energy(m);
-    const int de = max(-60, min(60, ei - ej));
-    const float pu = pow2i(de), pv = pow2i(-de);
-    // (u - E0) + (v - E0) is exact (Sterbenz) whenever the two models are similar -- exactly when it matters
-    float res = (fmaf(Shi_i, pu, -e.E0) + fmaf(Shi_j, pv, -e.E0))
-              + fmaf(2.0f, e.delta, fmaf(Slo_i, pu, Slo_j * pv));
-    res = res < 0.0f ? 0.0f : res;                                      // clamp (NaN stays NaN)
-    const int es = max(-120, min(120, ei + ej));
-    return sqrtf(res * invL * pow2i(es - es / 2) * pow2i(es / 2));
+    double c2 = 0.0;
+#pragma unroll
+    for (int i = 0; i < 9; ++i) c2 = fma(m[i], m[i], c2);
+    double C[9];
+    C[0] = m[4] * m[8] - m[5] * m[7];
+    C[1] = m[5] * m[6] - m[3] * m[8];
+    C[2] = m[3] * m[7] - m[4] * m[6];
+    C[3] = m[7] * m[2] - m[8] * m[1];
+    C[4] = m[8] * m[0] - m[6] * m[2];
+    C[5] = m[6] * m[1] - m[7] * m[0];
+    C[6] = m[1] * m[5] - m[2] * m[4];
+    C[7] = m[2] * m[3] - m[0] * m[5];
+    C[8] = m[0] * m[4] - m[1] * m[3];
+    double c1 = 0.0;
+#pragma unroll
+    for (int i = 0; i < 9; ++i) c1 = fma(C[i], C[i], c1);
+    const double d = m[0] * C[0] + m[1] * C[1] + m[2] * C[2];
+    // starting value: the fp32 closed form on the rounded invariants, rescaled into the fp32 range by a power of two
+    int e2 = 0;
+    (void)frexp(c2, &e2);
+    const int h = e2 / 2;                                             // c2 2^-2h in [0.25, 2)
+    EqInvariants<float> inv;
+    inv.c2 = (float)ldexp(c2, -2 * h);
+    inv.c1 = (float)ldexp(c1, -4 * h);
+    inv.d = (float)ldexp(d, -3 * h);
+    const EPair e0 = eq2_energy(inv);
+    double E = ldexp((double)e0.E0 - (double)e0.delta, h);
+    if (c2 > 0.0) {
+#pragma unroll
+        for (int it = 0; it < 2; ++it) {
+            const double t = fma(E, E, -c2);
+            const double f = fma(t, t, -8.0 * d * E - 4.0 * c1);
+            const double fp = 4.0 * E * t - 8.0 * d;
+            if (fp > 1e-6 * E * E * E) E -= f / fp;                   // s2 + S s3 -> 0: keep the deflated value
+        }
+    } else {
+        E = c2;                                                       // M == 0 -> 0; NaN stays NaN
+    }
+    const int de = max(-300, min(300, ei - ej));
+    double res = (ldexp(S_i, de) - E) + (ldexp(S_j, -de) - E);
+    res = res < 0.0 ? 0.0 : res;                                      // clamp (NaN stays NaN)
+    return (float)sqrt(ldexp(res * invL, ei + ej));
 }
 
 // The same last line when each model carries T = sum |a|^2 in its TRUE scale as two floats (Thi, Tlo) and

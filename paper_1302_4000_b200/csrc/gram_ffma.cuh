@@ -4,7 +4,10 @@
 // The nine sums of a pair are one 3x3 block of the product Y Y^T, Y = [3N x L] ("3x3
 // covariance matrix M" -- here for all pairs at once).  Each thread owns 2x2 pairs = a 6x6 register
 // block.  Accumulation is blocked: 16 atoms are summed into a fresh fp32 block, which is then added to
-// the running total, so no fp32 chain is longer than 16 + L/16 terms.
+// an FP64 running total, so no fp32 chain is longer than 16 terms; the closed form runs in FP64
+// (eq2_crmsd_f64).  This engine serves the chains too long for the tensor-core engine -- the most extended
+// inputs, whose R_g^2 every fp32 error term scales with -- so it spends its spare issue slots on accuracy
+// (DESIGN.md "Error budget").
 #pragma once
 #include "common.cuh"
 #include "epilogue.cuh"
@@ -76,9 +79,9 @@ gram_ffma_kernel(const float* __restrict__ Yt, const ModelStat* __restrict__ sta
         cp_async_commit();
     };
 
-    float tot[36];
+    double tot[36];
 #pragma unroll
-    for (int i = 0; i < 36; ++i) tot[i] = 0.0f;
+    for (int i = 0; i < 36; ++i) tot[i] = 0.0;
 
     const int nchunks = Lp16 / FF_KC;
     load_stage(0, 0);
@@ -111,7 +114,7 @@ gram_ffma_kernel(const float* __restrict__ Yt, const ModelStat* __restrict__ sta
                 for (int s = 0; s < 6; ++s) acc[6 * r + s] = fmaf(a[r], b[s], acc[6 * r + s]);
         }
 #pragma unroll
-        for (int i = 0; i < 36; ++i) tot[i] += acc[i];
+        for (int i = 0; i < 36; ++i) tot[i] += (double)acc[i];
         __syncthreads();
     }
 
@@ -127,12 +130,13 @@ gram_ffma_kernel(const float* __restrict__ Yt, const ModelStat* __restrict__ sta
             const int64_t j = j_base + 2 * cp + b;
             if (j >= N || j <= i) continue;
             const ModelStat sj = stats[j];
-            float m[9];
+            double m[9];
 #pragma unroll
             for (int p = 0; p < 3; ++p)
 #pragma unroll
                 for (int q = 0; q < 3; ++q) m[3 * p + q] = tot[6 * (3 * a + p) + 3 * b + q];
-            const float c = eq2_crmsd(m, si.Shi, si.Slo, si.ex, sj.Shi, sj.Slo, sj.ex, invL);
+            const float c = eq2_crmsd_f64(m, (double)si.Shi + (double)si.Slo, si.ex, (double)sj.Shi + (double)sj.Slo,
+                                          sj.ex, (double)invL);
             if (MODE == SINK_STORE) out[packed_index(i, j, N) - base] = c;
             else sink_emit<MODE>(sink, (int32_t)i, (int32_t)j, c);
         }
