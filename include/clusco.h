@@ -46,7 +46,8 @@
  *     same domain as the tensor-core engine.
  * Coordinates in other units scale these figures by the square of the unit.  Per-model scale exponents are clamped
  * to [-30, 30]: a model whose largest centred coordinate is >= 2^30 (or NaN/Inf) yields NaN for its pairs; a model
- * smaller than 2^-31 in every coordinate is treated as a point (its pairs get c^2 = R_other^2).  L <= 256 for the
+ * whose largest centred coordinate is below 2^-31 keeps the 2^-53 quantisation step (one bit of its 24 lost per
+ * factor of two).  L <= 256 for the
  * tensor-core engine (int32 level sums, A operand resident in tensor memory); N <= 2^24.
  */
 #ifndef CLUSCO_H

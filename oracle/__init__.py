@@ -356,6 +356,8 @@ def _load_g():
         lib = ctypes.CDLL(_compile(_SRC_G, _LIB_G, False))
         lib.oracle_gdt_pair.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p, _f64p]
         lib.oracle_gdt_pair.restype = None
+        lib.oracle_gdt_pair_trace.argtypes = [_f32p, _f32p, ctypes.c_int32, _f64p, _f64p, _i64p]
+        lib.oracle_gdt_pair_trace.restype = None
         lib.oracle_gdt_one_vs_all.argtypes = [_f32p, _f32p, ctypes.c_int64, ctypes.c_int32, _f64p]
         lib.oracle_gdt_one_vs_all.restype = None
         _lib_g = lib
@@ -370,6 +372,18 @@ def gdt_pair(ref, model):
     cnt = np.empty(4, np.float64)
     _load_g().oracle_gdt_pair(_p(a, _f32p), _p(b, _f32p), a.shape[0], _p(out, _f64p), _p(cnt, _f64p))
     return out, cnt
+
+
+def gdt_pair_trace(ref, model):
+    """gdt_pair plus the search-control diagnostics: (scores, counts, (seed fragments, superpositions evaluated in total,
+    most superpositions spent on one seed))."""
+    a, b = _f32(ref), _f32(model)
+    assert a.shape == b.shape
+    out = np.empty(3, np.float64)
+    cnt = np.empty(4, np.float64)
+    tr = np.zeros(3, np.int64)
+    _load_g().oracle_gdt_pair_trace(_p(a, _f32p), _p(b, _f32p), a.shape[0], _p(out, _f64p), _p(cnt, _f64p), _p(tr, _i64p))
+    return out, cnt, tuple(int(v) for v in tr)
 
 
 def gdt_one_vs_all(ref, coords):

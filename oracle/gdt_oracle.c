@@ -144,9 +144,12 @@ static int evaluate(const double *a, const double *b, int L, double R[3][3], con
 }
 
 /* One model against the reference: out[0] = GDT_TS (percent), out[1] = TM-score, out[2] = MaxSub;
-   out[3..6] (optional, counts != NULL) = max C_1, C_2, C_4, C_8. */
-void oracle_gdt_pair(const float *ref, const float *model, int32_t L, double *out, double *counts)
+   counts (optional) = max C_1, C_2, C_4, C_8;  trace (optional, diagnostics of the search control only -- no
+   arithmetic depends on it): trace[0] = number of seed fragments, trace[1] = superpositions evaluated in total,
+   trace[2] = most superpositions spent on one seed. */
+void oracle_gdt_pair_trace(const float *ref, const float *model, int32_t L, double *out, double *counts, int64_t *trace)
 {
+    int64_t n_seeds = 0, n_sup = 0, max_sup = 0;
     double *a = (double *)malloc(sizeof(double) * 3 * (size_t)L), *b = (double *)malloc(sizeof(double) * 3 * (size_t)L);
     unsigned char *sel = (unsigned char *)malloc((size_t)L);
     for (int i = 0; i < 3 * L; ++i) { a[i] = ref[i]; b[i] = model[i]; }
@@ -166,21 +169,32 @@ void oracle_gdt_pair(const float *ref, const float *model, int32_t L, double *ou
         for (int start = 0; start + len <= L; ++start) {
             for (int i = 0; i < L; ++i) sel[i] = i >= start && i < start + len;
             int prev = len, same = 0;
+            int64_t sup = 0;
             for (int it = 0; it < GDT_MAX_ITER; ++it) {
                 double R[3][3], t[3];
                 kabsch(a, b, sel, L, R, t);
                 int n = evaluate(a, b, L, R, t, d0, &best, sel);
+                ++sup;
                 if (n == prev) ++same; else same = 0;
                 prev = n;
                 if (same == 4 || n < 3) break;
             }
+            ++n_seeds;
+            n_sup += sup;
+            if (sup > max_sup) max_sup = sup;
         }
     }
+    if (trace) { trace[0] = n_seeds; trace[1] = n_sup; trace[2] = max_sup; }
     out[0] = 100.0 * 0.25 * (best.c[0] + best.c[1] + best.c[2] + best.c[3]) / (double)L;
     out[1] = best.tm;
     out[2] = best.maxsub;
     if (counts) for (int c = 0; c < 4; ++c) counts[c] = best.c[c];
     free(a); free(b); free(sel);
+}
+
+void oracle_gdt_pair(const float *ref, const float *model, int32_t L, double *out, double *counts)
+{
+    oracle_gdt_pair_trace(ref, model, L, out, counts, 0);
 }
 
 /* The reference against N models: out[3 n + {0,1,2}]. */
