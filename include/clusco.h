@@ -87,6 +87,15 @@ const char* clusco_version(void);
 int clusco_engine_supported(int engine, int32_t L);
 
 /*
+ * Host-only query: how the tensor-core engine decomposes an (N, L) all-pairs call -- out5 = { tiles of the upper
+ * triangle, 32-atom k-steps per tile, MMA columns issued per k-step and tile (all six digit products), row models
+ * per tile, column models per tile }.  One tile and k-step costs 128 rows x out5[2] columns x 32 atoms multiply-adds
+ * on the tensor pipe; bench.py derives the ISSUED work of its roofline from this (the ALGORITHMIC work is 9 L
+ * multiply-adds per pair).  CLUSCO_ERR_INVALID_ARG if the engine does not take L.
+ */
+int clusco_i8tc_geometry(int64_t N, int32_t L, int64_t* out5);
+
+/*
  * Centring and radius of gyration (implicit in eq. 2: M and R are taken about the centroid,
  * PAPER.md:40-45).   coords[N][L][3] -> centred[N][L][3] = x_i - mean(x)   (same layout; may alias
  * coords; may be NULL), r2[N] = (1/L) sum_i |x_i - mean|^2 = R^2 (may be NULL).
@@ -241,6 +250,21 @@ int clusco_gdt_allpairs(const float* coords, int64_t N, int32_t L, float* out, v
 int clusco_crmsd_allpairs_host(const float* coords_host, int64_t N, int32_t L, float* out_host);
 int clusco_crmsd_one_vs_all_host(const float* native_host, const float* coords_host, int64_t N,
                                  int32_t L, float* out_host);
+/*
+ * Host-buffer forms of the two fused consumers (the paper's first use case end to end, and the
+ * per-model reductions of PAPER.md:116): coordinates go up, only the triples / the per-model statistics come down --
+ * at C3 (10 000 x 250) 30 MB up and 18 MB down instead of the 200 MB matrix.  Semantics as
+ * clusco_crmsd_allpairs_below / clusco_crmsd_rowstats; every pointer is a HOST pointer (count_host too); blocking;
+ * same pool, lock and error behaviour as the calls above.  `capacity` may be a generous bound (up to N(N-1)/2): the
+ * device staging starts at 4 Mi triples and the compute stage is run a second time, with room for all, only when
+ * more pairs than that were found and the caller has room for them.  *count_host = number of pairs found (may exceed
+ * capacity: the first `capacity` triples are valid).
+ */
+int clusco_crmsd_allpairs_below_host(const float* coords_host, int64_t N, int32_t L, float cutoff, int64_t capacity,
+                                     int32_t* pair_i_host, int32_t* pair_j_host, float* pair_c_host,
+                                     unsigned long long* count_host);
+int clusco_crmsd_rowstats_host(const float* coords_host, int64_t N, int32_t L, float cutoff, double* rowsum_host,
+                               int32_t* below_host);
 /* Returns the pool kept by the *_host calls to the driver and destroys their streams (all devices). */
 int clusco_host_release(void);
 

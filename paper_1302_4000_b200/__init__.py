@@ -28,6 +28,7 @@ EXPORTS = (
     "clusco_host_release", "clusco_crmsd_allpairs_below", "clusco_crmsd_rowstats",
     "clusco_drmsd_allpairs_workspace", "clusco_drmsd_allpairs", "clusco_cmo_allpairs_workspace", "clusco_cmo_allpairs",
     "clusco_gdt_one_vs_all", "clusco_drmsd_one_vs_all", "clusco_cmo_one_vs_all", "clusco_gdt_allpairs",
+    "clusco_crmsd_allpairs_below_host", "clusco_crmsd_rowstats_host", "clusco_i8tc_geometry",
 )
 
 
@@ -80,6 +81,9 @@ def load(build_if_missing: bool = False):
     lib.clusco_drmsd_one_vs_all.argtypes = [vp, vp, i64, i32, vp, vp]
     lib.clusco_cmo_one_vs_all.argtypes = [vp, vp, i64, i32, ctypes.c_float, vp, vp]
     lib.clusco_gdt_allpairs.argtypes = [vp, i64, i32, vp, vp]
+    lib.clusco_crmsd_allpairs_below_host.argtypes = [vp, i64, i32, ctypes.c_float, i64, vp, vp, vp, vp]
+    lib.clusco_crmsd_rowstats_host.argtypes = [vp, i64, i32, ctypes.c_float, vp, vp]
+    lib.clusco_i8tc_geometry.argtypes = [i64, i32, ctypes.POINTER(ctypes.c_int64)]
     for name in EXPORTS:                       # every declared symbol must be exported
         getattr(lib, name)
     _lib = lib
@@ -116,12 +120,47 @@ def _check_coords(coords, name="coords"):
     return int(coords.shape[0]), int(coords.shape[1])
 
 
+def _check_buf(t, name, numel, dtype, device=None, cuda=True):
+    """A caller-supplied buffer goes to the library as a raw pointer: check everything the pointer cannot say."""
+    torch = _torch()
+    if not isinstance(t, torch.Tensor) or t.is_cuda != cuda or t.dtype != dtype or not t.is_contiguous() \
+            or t.numel() < numel or (cuda and device is not None and t.device != device):
+        where = f"CUDA (on {device})" if cuda else "host"
+        raise CluscoError(f"{name} must be a contiguous {where} {dtype} tensor with at least {numel} elements")
+    return t
+
+
+def _check_workspace(ws, nbytes, device):
+    torch = _torch()
+    if not isinstance(ws, torch.Tensor) or not ws.is_cuda or ws.device != device or not ws.is_contiguous() \
+            or ws.numel() * ws.element_size() < nbytes or ws.data_ptr() % 256:
+        raise CluscoError(f"workspace must be a contiguous CUDA tensor on {device} of at least {nbytes} bytes, "
+                          "256-byte aligned")
+    return ws
+
+
+def _check_host_coords(coords_host, name="coords_host"):
+    torch = _torch()
+    if not (isinstance(coords_host, torch.Tensor) and not coords_host.is_cuda and coords_host.dtype == torch.float32
+            and coords_host.dim() == 3 and coords_host.shape[2] == 3 and coords_host.is_contiguous()):
+        raise CluscoError(f"{name} must be a contiguous host float32 tensor of shape [N, L, 3]")
+    return int(coords_host.shape[0]), int(coords_host.shape[1])
+
+
 def version() -> str:
     return load().clusco_version().decode()
 
 
 def engine_supported(engine: int, L: int) -> bool:
     return bool(load().clusco_engine_supported(engine, L))
+
+
+def i8tc_geometry(N: int, L: int) -> dict:
+    """The tensor-core engine's work decomposition for (N, L) (include/clusco.h: clusco_i8tc_geometry)."""
+    o = (ctypes.c_int64 * 5)()
+    _check(load().clusco_i8tc_geometry(N, L, o), "clusco_i8tc_geometry")
+    return {"tiles": int(o[0]), "ksteps": int(o[1]), "mma_columns_per_kstep": int(o[2]), "row_models": int(o[3]),
+            "col_models": int(o[4])}
 
 
 def n_pairs(N: int) -> int:
@@ -136,6 +175,8 @@ def clusco_center(coords, centred=None, r2=None):
         centred = torch.empty_like(coords)
     if r2 is None:
         r2 = torch.empty(N, dtype=torch.float32, device=coords.device)
+    _check_buf(centred, "centred", N * L * 3, torch.float32, coords.device)
+    _check_buf(r2, "r2", N, torch.float32, coords.device)
     with torch.cuda.device(coords.device):
         _check(load().clusco_center(_ptr(coords), N, L, _ptr(centred), _ptr(r2), _stream_ptr(coords)),
                "clusco_center")
@@ -154,11 +195,15 @@ def clusco_crmsd_allpairs(coords, out=None, workspace=None, engine: int = ENGINE
     row_end = N if row_end is None else row_end
     lo = row_begin * (2 * N - row_begin - 1) // 2
     hi = row_end * (2 * N - row_end - 1) // 2
+    if not (0 <= row_begin <= row_end <= N):
+        raise CluscoError("need 0 <= row_begin <= row_end <= N")
     if out is None:
         out = torch.empty(max(hi - lo, 0), dtype=torch.float32, device=coords.device)
     nbytes = clusco_crmsd_allpairs_workspace(N, L)
     if workspace is None:
         workspace = torch.empty(nbytes, dtype=torch.uint8, device=coords.device)
+    _check_buf(out, "out", max(hi - lo, 0), torch.float32, coords.device)
+    _check_workspace(workspace, nbytes, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_crmsd_allpairs_ex(_ptr(coords), N, L, row_begin, row_end, _ptr(out), _ptr(workspace),
                                              workspace.numel() * workspace.element_size(), engine,
@@ -171,6 +216,7 @@ def clusco_allpairs_prepare(coords, workspace, engine: int = ENGINE_AUTO):
     """Stage 1 of the all-pairs call (centring, R^2, operand planes) into `workspace`."""
     torch = _torch()
     N, L = _check_coords(coords)
+    _check_workspace(workspace, clusco_crmsd_allpairs_workspace(N, L), coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_allpairs_prepare(_ptr(coords), N, L, _ptr(workspace),
                                             workspace.numel() * workspace.element_size(), engine,
@@ -183,6 +229,13 @@ def clusco_allpairs_compute(N: int, L: int, out, workspace, engine: int = ENGINE
     """Stage 2 of the all-pairs call (Gram + eq. 2 + packed store) from a prepared workspace."""
     torch = _torch()
     row_end = N if row_end is None else row_end
+    if not (0 <= row_begin <= row_end <= N):
+        raise CluscoError("need 0 <= row_begin <= row_end <= N")
+    need = row_end * (2 * N - row_end - 1) // 2 - row_begin * (2 * N - row_begin - 1) // 2
+    if not (isinstance(out, torch.Tensor) and out.is_cuda):
+        raise CluscoError("out must be a CUDA tensor")
+    _check_buf(out, "out", need, torch.float32, out.device)
+    _check_workspace(workspace, clusco_crmsd_allpairs_workspace(N, L), out.device)
     with torch.cuda.device(out.device):
         st = load().clusco_allpairs_compute(N, L, row_begin, row_end, _ptr(out), _ptr(workspace),
                                             workspace.numel() * workspace.element_size(), engine,
@@ -203,6 +256,7 @@ def clusco_crmsd_allpairs_below(coords, cutoff: float, capacity: int, workspace=
     count = torch.empty(1, dtype=torch.int64, device=dev)
     if workspace is None:
         workspace = torch.empty(clusco_crmsd_allpairs_workspace(N, L), dtype=torch.uint8, device=dev)
+    _check_workspace(workspace, clusco_crmsd_allpairs_workspace(N, L), dev)
     with torch.cuda.device(dev):
         st = load().clusco_crmsd_allpairs_below(_ptr(coords), N, L, float(cutoff), capacity, _ptr(pi), _ptr(pj), _ptr(pc),
                                                 _ptr(count), _ptr(workspace),
@@ -220,6 +274,7 @@ def clusco_crmsd_rowstats(coords, cutoff: float, workspace=None):
     below = torch.empty(N, dtype=torch.int32, device=dev)
     if workspace is None:
         workspace = torch.empty(clusco_crmsd_allpairs_workspace(N, L), dtype=torch.uint8, device=dev)
+    _check_workspace(workspace, clusco_crmsd_allpairs_workspace(N, L), dev)
     with torch.cuda.device(dev):
         st = load().clusco_crmsd_rowstats(_ptr(coords), N, L, float(cutoff), _ptr(rowsum), _ptr(below), _ptr(workspace),
                                           workspace.numel() * workspace.element_size(), _stream_ptr(coords))
@@ -233,9 +288,11 @@ def clusco_drmsd_allpairs(coords, out=None, workspace=None):
     N, L = _check_coords(coords)
     if out is None:
         out = torch.empty(n_pairs(N), dtype=torch.float32, device=coords.device)
+    nbytes = int(load().clusco_drmsd_allpairs_workspace(N, L))
     if workspace is None:
-        nbytes = int(load().clusco_drmsd_allpairs_workspace(N, L))
         workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=coords.device)
+    _check_buf(out, "out", n_pairs(N), torch.float32, coords.device)
+    _check_workspace(workspace, nbytes, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_drmsd_allpairs(_ptr(coords), N, L, _ptr(out), _ptr(workspace),
                                           workspace.numel() * workspace.element_size(), _stream_ptr(coords))
@@ -249,9 +306,11 @@ def clusco_cmo_allpairs(coords, cutoff: float, out=None, workspace=None):
     N, L = _check_coords(coords)
     if out is None:
         out = torch.empty(n_pairs(N), dtype=torch.float32, device=coords.device)
+    nbytes = int(load().clusco_cmo_allpairs_workspace(N, L))
     if workspace is None:
-        nbytes = int(load().clusco_cmo_allpairs_workspace(N, L))
         workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=coords.device)
+    _check_buf(out, "out", n_pairs(N), torch.float32, coords.device)
+    _check_workspace(workspace, nbytes, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_cmo_allpairs(_ptr(coords), N, L, float(cutoff), _ptr(out), _ptr(workspace),
                                         workspace.numel() * workspace.element_size(), _stream_ptr(coords))
@@ -268,6 +327,7 @@ def clusco_crmsd_one_vs_all(native, coords, out=None):
         raise CluscoError("native must be a contiguous CUDA float32 tensor of shape [L, 3]")
     if out is None:
         out = torch.empty(N, dtype=torch.float32, device=coords.device)
+    _check_buf(out, "out", N, torch.float32, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_crmsd_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_crmsd_one_vs_all")
@@ -289,6 +349,7 @@ def clusco_drmsd_one_vs_all(native, coords, out=None):
     N, L = _check_native(native, coords)
     if out is None:
         out = torch.empty(N, dtype=torch.float32, device=coords.device)
+    _check_buf(out, "out", N, torch.float32, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_drmsd_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_drmsd_one_vs_all")
@@ -301,6 +362,7 @@ def clusco_cmo_one_vs_all(native, coords, cutoff: float, out=None):
     N, L = _check_native(native, coords)
     if out is None:
         out = torch.empty(N, dtype=torch.float32, device=coords.device)
+    _check_buf(out, "out", N, torch.float32, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_cmo_one_vs_all(_ptr(native), _ptr(coords), N, L, float(cutoff), _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_cmo_one_vs_all")
@@ -316,6 +378,7 @@ def clusco_gdt_one_vs_all(native, coords, out=None):
         raise CluscoError("native must be a contiguous CUDA float32 tensor of shape [L, 3]")
     if out is None:
         out = torch.empty((N, 3), dtype=torch.float32, device=coords.device)
+    _check_buf(out, "out", 3 * N, torch.float32, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_gdt_one_vs_all(_ptr(native), _ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_gdt_one_vs_all")
@@ -328,6 +391,7 @@ def clusco_gdt_allpairs(coords, out=None):
     N, L = _check_coords(coords)
     if out is None:
         out = torch.empty((n_pairs(N), 3), dtype=torch.float32, device=coords.device)
+    _check_buf(out, "out", 3 * n_pairs(N), torch.float32, coords.device)
     with torch.cuda.device(coords.device):
         st = load().clusco_gdt_allpairs(_ptr(coords), N, L, _ptr(out), _stream_ptr(coords))
     _check(st, "clusco_gdt_allpairs")
@@ -337,10 +401,10 @@ def clusco_gdt_allpairs(coords, out=None):
 def clusco_crmsd_allpairs_host(coords_host, out_host=None):
     """Host-buffer call (blocking): CPU float32 tensors in and out; copies are inside the call."""
     torch = _torch()
-    assert coords_host.dtype == torch.float32 and not coords_host.is_cuda and coords_host.is_contiguous()
-    N, L = int(coords_host.shape[0]), int(coords_host.shape[1])
+    N, L = _check_host_coords(coords_host)
     if out_host is None:
         out_host = torch.empty(n_pairs(N), dtype=torch.float32, pin_memory=True)
+    _check_buf(out_host, "out_host", n_pairs(N), torch.float32, cuda=False)
     _check(load().clusco_crmsd_allpairs_host(_ptr(coords_host), N, L, _ptr(out_host)),
            "clusco_crmsd_allpairs_host")
     return out_host
@@ -348,12 +412,52 @@ def clusco_crmsd_allpairs_host(coords_host, out_host=None):
 
 def clusco_crmsd_one_vs_all_host(native_host, coords_host, out_host=None):
     torch = _torch()
-    N, L = int(coords_host.shape[0]), int(coords_host.shape[1])
+    N, L = _check_host_coords(coords_host)
+    if not (isinstance(native_host, torch.Tensor) and not native_host.is_cuda and native_host.dtype == torch.float32
+            and tuple(native_host.shape) == (L, 3) and native_host.is_contiguous()):
+        raise CluscoError("native_host must be a contiguous host float32 tensor of shape [L, 3]")
     if out_host is None:
         out_host = torch.empty(N, dtype=torch.float32, pin_memory=True)
+    _check_buf(out_host, "out_host", N, torch.float32, cuda=False)
     _check(load().clusco_crmsd_one_vs_all_host(_ptr(native_host), _ptr(coords_host), N, L, _ptr(out_host)),
            "clusco_crmsd_one_vs_all_host")
     return out_host
+
+
+def clusco_crmsd_allpairs_below_host(coords_host, cutoff: float, capacity: int, out=None):
+    """Host-buffer form of clusco_crmsd_allpairs_below (blocking): returns (pair_i int32[capacity], pair_j, pair_c
+    float32 -- host tensors -- and the count as a Python int); the first min(count, capacity) slots are valid."""
+    torch = _torch()
+    N, L = _check_host_coords(coords_host)
+    if capacity < 0:
+        raise CluscoError("capacity must be >= 0")
+    if out is None:
+        out = (torch.empty(capacity, dtype=torch.int32, pin_memory=capacity > 0),
+               torch.empty(capacity, dtype=torch.int32, pin_memory=capacity > 0),
+               torch.empty(capacity, dtype=torch.float32, pin_memory=capacity > 0))
+    pi, pj, pc = out
+    _check_buf(pi, "pair_i", capacity, torch.int32, cuda=False)
+    _check_buf(pj, "pair_j", capacity, torch.int32, cuda=False)
+    _check_buf(pc, "pair_c", capacity, torch.float32, cuda=False)
+    count = ctypes.c_ulonglong(0)
+    _check(load().clusco_crmsd_allpairs_below_host(_ptr(coords_host), N, L, float(cutoff), capacity, _ptr(pi), _ptr(pj),
+                                                   _ptr(pc), ctypes.cast(ctypes.byref(count), ctypes.c_void_p)),
+           "clusco_crmsd_allpairs_below_host")
+    return pi, pj, pc, int(count.value)
+
+
+def clusco_crmsd_rowstats_host(coords_host, cutoff: float, out=None):
+    """Host-buffer form of clusco_crmsd_rowstats (blocking): (rowsum float64[N], below int32[N]) host tensors."""
+    torch = _torch()
+    N, L = _check_host_coords(coords_host)
+    if out is None:
+        out = (torch.empty(N, dtype=torch.float64, pin_memory=N > 0), torch.empty(N, dtype=torch.int32, pin_memory=N > 0))
+    rowsum, below = out
+    _check_buf(rowsum, "rowsum", N, torch.float64, cuda=False)
+    _check_buf(below, "below", N, torch.int32, cuda=False)
+    _check(load().clusco_crmsd_rowstats_host(_ptr(coords_host), N, L, float(cutoff), _ptr(rowsum), _ptr(below)),
+           "clusco_crmsd_rowstats_host")
+    return rowsum, below
 
 
 def clusco_host_release():

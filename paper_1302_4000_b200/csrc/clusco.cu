@@ -67,6 +67,22 @@ int clusco_engine_supported(int engine, int32_t L)
     return 0;
 }
 
+int clusco_i8tc_geometry(int64_t N, int32_t L, int64_t* out5)
+{
+    if (N < 0 || L < 1 || !out5 || !i8tc_supported(L)) return CLUSCO_ERR_INVALID_ARG;
+    const Workspace w = workspace_layout(N, L);
+    I8Tiles t;
+    t.Tc = w.col_tiles;
+    t.I_lo = 0;
+    t.I_hi = w.row_tiles;
+    out5[0] = N < 2 ? 0 : i8_tiles_before(t, t.I_hi);
+    out5[1] = w.Lp32 / 32;
+    out5[2] = 6 * 3 * I8_COL_MODELS;                         // six digit products x (3 components x column models)
+    out5[3] = I8_ROW_MODELS;
+    out5[4] = I8_COL_MODELS;
+    return CLUSCO_OK;
+}
+
 int clusco_center(const float* coords, int64_t N, int32_t L, float* centred, float* r2, void* stream)
 {
     if (N < 0 || L < 1) return CLUSCO_ERR_INVALID_ARG;
@@ -443,12 +459,13 @@ struct HostCtx {
 std::mutex g_host_mu;
 HostCtx g_host[64];
 
-int host_ctx(HostCtx** out)
+// the caller holds g_host_mu (and keeps it for the whole host call, so that clusco_host_release() cannot destroy the
+// pool and the streams under a running call)
+int host_ctx_locked(HostCtx** out)
 {
     int dev = 0;
     CLUSCO_CUDA_TRY(cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) return CLUSCO_ERR_INVALID_ARG;
-    std::lock_guard<std::mutex> lock(g_host_mu);
     HostCtx& c = g_host[dev];
     if (!c.pool) {
         cudaMemPoolProps props;
@@ -508,10 +525,10 @@ int clusco_crmsd_allpairs_host(const float* coords_host, int64_t N, int32_t L, f
     if (!coords_host || !out_host) return CLUSCO_ERR_INVALID_ARG;
     int st = check_device(nullptr);
     if (st != CLUSCO_OK) return st;
-    HostCtx* ctx = nullptr;
-    st = host_ctx(&ctx);
-    if (st != CLUSCO_OK) return st;
     std::lock_guard<std::mutex> lock(g_host_mu);             // one host call at a time per process
+    HostCtx* ctx = nullptr;
+    st = host_ctx_locked(&ctx);
+    if (st != CLUSCO_OK) return st;
     const size_t in_bytes = (size_t)N * L * 3 * sizeof(float);
     const size_t n_pairs = (size_t)N * (size_t)(N - 1) / 2;
     const size_t ws_bytes = clusco_crmsd_allpairs_workspace(N, L);
@@ -566,10 +583,10 @@ int clusco_crmsd_one_vs_all_host(const float* native_host, const float* coords_h
     if (!native_host || !coords_host || !out_host) return CLUSCO_ERR_INVALID_ARG;
     int st = check_device(nullptr);
     if (st != CLUSCO_OK) return st;
-    HostCtx* ctx = nullptr;
-    st = host_ctx(&ctx);
-    if (st != CLUSCO_OK) return st;
     std::lock_guard<std::mutex> lock(g_host_mu);
+    HostCtx* ctx = nullptr;
+    st = host_ctx_locked(&ctx);
+    if (st != CLUSCO_OK) return st;
     const size_t model_bytes = (size_t)L * 3 * sizeof(float);
     cudaStream_t sc = ctx->compute, sx = ctx->copy;
     float *d_in = nullptr, *d_nat = nullptr, *d_out = nullptr;
@@ -606,6 +623,128 @@ int clusco_crmsd_one_vs_all_host(const float* native_host, const float* coords_h
     if (d_in) cudaFreeAsync(d_in, sc);
     if (d_nat) cudaFreeAsync(d_nat, sc);
     if (d_out) cudaFreeAsync(d_out, sc);
+    return err.st;
+}
+
+// ---- host-buffer forms of the fused consumers: the coordinates go up, only the triples / the
+// per-model statistics come down -- 18 MB instead of the 200 MB matrix at C3 ---------------------------------------
+int clusco_crmsd_allpairs_below_host(const float* coords_host, int64_t N, int32_t L, float cutoff, int64_t capacity,
+                                     int32_t* pair_i_host, int32_t* pair_j_host, float* pair_c_host,
+                                     unsigned long long* count_host)
+{
+    if (N < 0 || L < 1 || capacity < 0 || !count_host) return CLUSCO_ERR_INVALID_ARG;
+    if (capacity > 0 && (!pair_i_host || !pair_j_host || !pair_c_host)) return CLUSCO_ERR_INVALID_ARG;
+    *count_host = 0ull;
+    if (N < 2) return CLUSCO_OK;
+    if (!coords_host) return CLUSCO_ERR_INVALID_ARG;
+    int st = check_device(nullptr);
+    if (st != CLUSCO_OK) return st;
+    std::lock_guard<std::mutex> lock(g_host_mu);
+    HostCtx* ctx = nullptr;
+    st = host_ctx_locked(&ctx);
+    if (st != CLUSCO_OK) return st;
+    const size_t in_bytes = (size_t)N * L * 3 * sizeof(float);
+    const size_t ws_bytes = clusco_crmsd_allpairs_workspace(N, L);
+    const int64_t n_pairs = N * (N - 1) / 2;
+    cudaStream_t sc = ctx->compute;
+    float* d_in = nullptr;
+    void* d_ws = nullptr;
+    unsigned long long* d_count = nullptr;
+    char* d_tri = nullptr;                                   // [pair_i | pair_j | pair_c], dev_cap entries each
+    ErrLatch err;
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_in, in_bytes, ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync(&d_ws, ws_bytes, ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_count, sizeof(unsigned long long), ctx->pool, sc));
+    // the caller's capacity may be a worst-case bound (all N(N-1)/2 pairs); the device staging starts at 4 Mi triples
+    // and a second pass of the compute stage follows only if the count says more are wanted AND the caller has room
+    int64_t dev_cap = capacity < n_pairs ? capacity : n_pairs;
+    if (dev_cap > ((int64_t)1 << 22)) dev_cap = (int64_t)1 << 22;
+    unsigned long long found = 0ull;
+    if (err.ok()) err.cuda(cudaMemcpyAsync(d_in, coords_host, in_bytes, cudaMemcpyHostToDevice, sc));
+    for (int pass = 0; pass < 2 && err.ok(); ++pass) {
+        if (dev_cap > 0) err.cuda(cudaMallocFromPoolAsync((void**)&d_tri, (size_t)dev_cap * 12, ctx->pool, sc));
+        if (!err.ok()) break;
+        int32_t* d_i = (int32_t*)d_tri;
+        int32_t* d_j = d_i + dev_cap;
+        float* d_c = (float*)(d_j + dev_cap);
+        if (pass == 0) {
+            err.status(clusco_crmsd_allpairs_below(d_in, N, L, cutoff, dev_cap, d_i, d_j, d_c, d_count, d_ws, ws_bytes,
+                                                   (void*)sc));
+        } else {                                             // the workspace is still prepared: compute stage only
+            err.cuda(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), sc));
+            Sink sink{};
+            sink.cutoff = cutoff;
+            sink.capacity = dev_cap;
+            sink.pair_i = d_i;
+            sink.pair_j = d_j;
+            sink.pair_c = d_c;
+            sink.count = d_count;
+            err.status(allpairs_compute_mode<SINK_BELOW>(N, L, 0, N, nullptr, sink, d_ws, ws_bytes, CLUSCO_ENGINE_AUTO,
+                                                         (void*)sc));
+        }
+        if (!err.ok()) break;
+        err.cuda(cudaMemcpyAsync(&found, d_count, sizeof(found), cudaMemcpyDeviceToHost, sc));
+        err.cuda(cudaStreamSynchronize(sc));
+        if (!err.ok()) break;
+        const int64_t want = (int64_t)found < capacity ? (int64_t)found : capacity;
+        if (want <= dev_cap) {
+            if (want > 0) {
+                err.cuda(cudaMemcpyAsync(pair_i_host, d_i, (size_t)want * 4, cudaMemcpyDeviceToHost, sc));
+                err.cuda(cudaMemcpyAsync(pair_j_host, d_j, (size_t)want * 4, cudaMemcpyDeviceToHost, sc));
+                err.cuda(cudaMemcpyAsync(pair_c_host, d_c, (size_t)want * 4, cudaMemcpyDeviceToHost, sc));
+            }
+            break;
+        }
+        cudaFreeAsync(d_tri, sc);                            // more wanted than staged: once more with room for all
+        d_tri = nullptr;
+        dev_cap = want;
+    }
+    err.cuda(cudaStreamSynchronize(sc));
+    if (err.ok()) *count_host = found;
+    if (d_tri) cudaFreeAsync(d_tri, sc);
+    if (d_count) cudaFreeAsync(d_count, sc);
+    if (d_in) cudaFreeAsync(d_in, sc);
+    if (d_ws) cudaFreeAsync(d_ws, sc);
+    return err.st;
+}
+
+int clusco_crmsd_rowstats_host(const float* coords_host, int64_t N, int32_t L, float cutoff, double* rowsum_host,
+                               int32_t* below_host)
+{
+    if (N < 0 || L < 1) return CLUSCO_ERR_INVALID_ARG;
+    if (N == 0) return CLUSCO_OK;
+    if (!coords_host || !rowsum_host || !below_host) return CLUSCO_ERR_INVALID_ARG;
+    int st = check_device(nullptr);
+    if (st != CLUSCO_OK) return st;
+    std::lock_guard<std::mutex> lock(g_host_mu);
+    HostCtx* ctx = nullptr;
+    st = host_ctx_locked(&ctx);
+    if (st != CLUSCO_OK) return st;
+    const size_t in_bytes = (size_t)N * L * 3 * sizeof(float);
+    const size_t ws_bytes = clusco_crmsd_allpairs_workspace(N, L);
+    cudaStream_t sc = ctx->compute;
+    float* d_in = nullptr;
+    void* d_ws = nullptr;
+    double* d_sum = nullptr;
+    int32_t* d_below = nullptr;
+    ErrLatch err;
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_in, in_bytes, ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync(&d_ws, ws_bytes, ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_sum, (size_t)N * sizeof(double), ctx->pool, sc));
+    err.cuda(cudaMallocFromPoolAsync((void**)&d_below, (size_t)N * sizeof(int32_t), ctx->pool, sc));
+    if (err.ok()) {
+        err.cuda(cudaMemcpyAsync(d_in, coords_host, in_bytes, cudaMemcpyHostToDevice, sc));
+        err.status(clusco_crmsd_rowstats(d_in, N, L, cutoff, d_sum, d_below, d_ws, ws_bytes, (void*)sc));
+    }
+    if (err.ok()) {
+        err.cuda(cudaMemcpyAsync(rowsum_host, d_sum, (size_t)N * sizeof(double), cudaMemcpyDeviceToHost, sc));
+        err.cuda(cudaMemcpyAsync(below_host, d_below, (size_t)N * sizeof(int32_t), cudaMemcpyDeviceToHost, sc));
+    }
+    err.cuda(cudaStreamSynchronize(sc));
+    if (d_in) cudaFreeAsync(d_in, sc);
+    if (d_ws) cudaFreeAsync(d_ws, sc);
+    if (d_sum) cudaFreeAsync(d_sum, sc);
+    if (d_below) cudaFreeAsync(d_below, sc);
     return err.st;
 }
 

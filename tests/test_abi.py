@@ -62,6 +62,43 @@ def test_argument_validation_needs_no_gpu(lib):
     assert lib.clusco_crmsd_one_vs_all(None, None, 3, 10, None, None) == 1
 
 
+def test_host_consumer_calls_validate_without_a_gpu(lib):
+    i64, i32, vp, f = ctypes.c_int64, ctypes.c_int32, ctypes.c_void_p, ctypes.c_float
+    lib.clusco_crmsd_allpairs_below_host.argtypes = [vp, i64, i32, f, i64, vp, vp, vp, vp]
+    lib.clusco_crmsd_rowstats_host.argtypes = [vp, i64, i32, f, vp, vp]
+    count = ctypes.c_ulonglong(7)
+    cp = ctypes.cast(ctypes.byref(count), vp)
+    assert lib.clusco_crmsd_allpairs_below_host(None, 1, 10, 3.2, 0, None, None, None, cp) == 0 and count.value == 0
+    assert lib.clusco_crmsd_allpairs_below_host(None, 5, 10, 3.2, 0, None, None, None, None) == 1     # no count
+    assert lib.clusco_crmsd_allpairs_below_host(None, 5, 10, 3.2, 4, None, None, None, cp) == 1       # capacity, no arrays
+    assert lib.clusco_crmsd_allpairs_below_host(None, 5, 0, 3.2, 0, None, None, None, cp) == 1
+    assert lib.clusco_crmsd_rowstats_host(None, 0, 10, 3.2, None, None) == 0
+    assert lib.clusco_crmsd_rowstats_host(None, 5, 10, 3.2, None, None) == 1
+    assert lib.clusco_crmsd_rowstats_host(None, -1, 10, 3.2, None, None) == 1
+
+
+def test_binding_rejects_bad_buffers_before_the_library_sees_them():
+    """The binding passes raw pointers: a short, wrong-dtype, non-contiguous or host tensor must raise, not corrupt memory.
+    (Checked on host tensors: the checks run before any device work.)"""
+    import torch
+    import paper_1302_4000_b200 as pkg
+    x = torch.zeros((4, 5, 3), dtype=torch.float32)
+    with pytest.raises(pkg.CluscoError):
+        pkg.clusco_crmsd_allpairs(x)                                   # not a CUDA tensor
+    with pytest.raises(pkg.CluscoError):
+        pkg.clusco_crmsd_allpairs_host(x.double())
+    with pytest.raises(pkg.CluscoError):
+        pkg.clusco_crmsd_allpairs_host(x, torch.zeros(3))              # needs 6 results
+    with pytest.raises(pkg.CluscoError):
+        pkg.clusco_crmsd_allpairs_host(x[:, :, :2])
+    with pytest.raises(pkg.CluscoError):
+        pkg.clusco_crmsd_one_vs_all_host(torch.zeros((4, 3)), x)        # native of the wrong length
+    with pytest.raises(pkg.CluscoError):
+        pkg.clusco_crmsd_rowstats_host(x, 3.0, out=(torch.zeros(4), torch.zeros(4, dtype=torch.int32)))   # float32 sums
+    with pytest.raises(pkg.CluscoError):
+        pkg.clusco_crmsd_allpairs_below_host(x, 3.0, 8, out=(torch.zeros(8, dtype=torch.int32),) * 3)
+
+
 def test_partition_rows(lib):
     import paper_1302_4000_b200 as pkg
     for N, parts in ((10000, 2), (30000, 8), (200, 4), (1000, 1)):

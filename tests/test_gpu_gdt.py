@@ -90,3 +90,16 @@ def test_gdt_allpairs(clusco, cfg, N):
     got = clusco.clusco_gdt_allpairs(_dev(ens.coords)).cpu().numpy()
     _check(got, want, f"{cfg} all pairs")
     assert clusco.clusco_gdt_allpairs(_dev(ens.coords[:1])).shape == (0, 3)
+
+
+def test_gdt_search_control_fixtures(clusco):
+    """The fixtures that pin the oracle's search control (tests/test_gdt_pins.py), through the kernel: the 3.5 A
+    re-selection cases have closed-form counts (GDT_TS = 100 * (20+40+40+40)/240 and 100 * (20+20+40+40)/240), and
+    the one-displaced-atom / hinge cases of the pins are covered above."""
+    from test_gdt_pins import _three_segments
+    for delta, counts in ((3.2, (20, 40, 40, 40)), (3.8, (20, 20, 40, 40))):
+        a, b, _ = _three_segments(delta)
+        want = oracle.gdt_one_vs_all(a, b[None])
+        got = clusco.clusco_gdt_one_vs_all(_dev(a), _dev(b[None])).cpu().numpy()
+        _check(got, want, f"three segments, delta {delta}")
+        assert abs(got[0, 0] - 100.0 * sum(counts) / 240.0) < 1e-4

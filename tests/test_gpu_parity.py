@@ -418,3 +418,60 @@ def test_consumers_edge_cases(clusco):
     assert torch.isnan(rs).all() and int(bl[5]) == 0 and int(bl[0]) == 62
     pi, pj, pc, count = clusco.clusco_crmsd_allpairs_below(y, 1e9, 64 * 63 // 2)
     assert int(count.item()) == 63 * 62 // 2
+
+
+def test_consumer_host_calls(clusco):
+    """The host-buffer forms return what the device-pointer forms return (same kernels): pinned and pageable memory,
+    a capacity smaller than the count, and the second pass that follows when more than the 4 Mi staged triples are found."""
+    import torch
+    ens = wl.make_config("C3", N=700)
+    x_h = torch.from_numpy(ens.coords)
+    x_d = _dev(ens.coords)
+    N = ens.N
+    rs_d, bl_d = clusco.clusco_crmsd_rowstats(x_d, 3.2)
+    for pin in (True, False):
+        rs_h, bl_h = clusco.clusco_crmsd_rowstats_host(x_h.pin_memory() if pin else x_h, 3.2)
+        assert torch.equal(bl_h, bl_d.cpu()) and float((rs_h - rs_d.cpu()).abs().max()) < 1e-9 * N
+    pi, pj, pc, count = clusco.clusco_crmsd_allpairs_below(x_d, 3.2, N * (N - 1) // 2)
+    n = int(count.item())
+    want = dict(zip(wl.packed_index(pi[:n].cpu().numpy().astype(np.int64), pj[:n].cpu().numpy().astype(np.int64), N).tolist(),
+                    pc[:n].cpu().numpy().tolist()))
+    hi, hj, hc, n_h = clusco.clusco_crmsd_allpairs_below_host(x_h, 3.2, N * (N - 1) // 2)
+    assert n_h == n and n > 1000
+    got = dict(zip(wl.packed_index(hi[:n].numpy().astype(np.int64), hj[:n].numpy().astype(np.int64), N).tolist(),
+                   hc[:n].numpy().tolist()))
+    assert got == want
+    hi, hj, hc, n_h = clusco.clusco_crmsd_allpairs_below_host(x_h, 3.2, 100)        # capacity below the count
+    assert n_h == n
+    k = wl.packed_index(hi.numpy().astype(np.int64), hj.numpy().astype(np.int64), N).tolist()
+    assert len(set(k)) == 100 and all(want[a] == c for a, c in zip(k, hc.numpy().tolist()))
+    assert clusco.clusco_crmsd_allpairs_below_host(x_h, 3.2, 0)[3] == n                # count only
+    assert clusco.clusco_crmsd_allpairs_below_host(x_h[:1], 3.2, 4)[3] == 0
+    # more hits than the 4 Mi staged triples: C2's first 3100 models below 1e9 A = all 4 803 450 pairs
+    big = wl.make_config("C2", N=3100)
+    P = big.N * (big.N - 1) // 2
+    hi, hj, hc, n_h = clusco.clusco_crmsd_allpairs_below_host(torch.from_numpy(big.coords), 1e9, P)
+    assert n_h == P > (1 << 22)
+    k = wl.packed_index(hi.numpy().astype(np.int64), hj.numpy().astype(np.int64), big.N)
+    assert np.array_equal(np.sort(k), np.arange(P))
+    ref = clusco.clusco_crmsd_allpairs(_dev(big.coords)).cpu().numpy()
+    assert np.array_equal(hc.numpy(), ref[k])
+    clusco.clusco_host_release()
+
+
+def test_binding_rejects_bad_device_buffers(clusco):
+    import torch
+    x = _dev(wl.make_config("C1").coords)
+    N = x.shape[0]
+    with pytest.raises(clusco.CluscoError):
+        clusco.clusco_crmsd_allpairs(x, out=torch.empty(10, device="cuda"))                     # too short
+    with pytest.raises(clusco.CluscoError):
+        clusco.clusco_crmsd_allpairs(x, out=torch.empty(N * (N - 1) // 2, dtype=torch.float64, device="cuda"))
+    with pytest.raises(clusco.CluscoError):
+        clusco.clusco_crmsd_allpairs(x, out=torch.empty(N * (N - 1) // 2))                      # host tensor
+    with pytest.raises(clusco.CluscoError):
+        clusco.clusco_crmsd_allpairs(x, workspace=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(clusco.CluscoError):
+        clusco.clusco_crmsd_one_vs_all(x[0].contiguous(), x, out=torch.empty(N - 1, device="cuda"))
+    with pytest.raises(clusco.CluscoError):
+        clusco.clusco_drmsd_allpairs(x, out=torch.empty((N * (N - 1) // 2, 2), device="cuda")[:, 0])   # not contiguous

@@ -56,6 +56,16 @@ def _rank_main(rank, world, port, N, q):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         assert float(t) == float(world)
 
+        # bench.py's own N > 1 code path (`--gpus N` = ONE ensemble, row-partitioned): the slice each rank times and
+        # the per-rank record of the JSON line, driven here with gloo and host tensors
+        import bench
+        bounds, lo2, hi2, my_pairs = bench.rank_slice(pkg, N, world, rank)
+        assert (lo2, hi2) == (lo, hi) and my_pairs == end - base
+        job_ms, per_rank = bench.combine_ranks(torch, dist, world, bounds, 10.0 + rank, 9.0 + rank, my_pairs, "cpu")
+        assert job_ms == 10.0 + world - 1 and sum(per_rank["pairs"]) == P
+        assert per_rank["rows"][0][0] == 0 and per_rank["rows"][-1][1] == N
+        assert abs(per_rank["slowest_over_fastest"] - (10.0 + world - 1) / 10.0) < 1e-12
+
         # check-only gather: concatenated slices == the full triangle
         parts = [None] * world
         dist.all_gather_object(parts, mine.astype(np.float64))
