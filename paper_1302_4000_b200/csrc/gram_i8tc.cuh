@@ -19,12 +19,16 @@
 // every epilogue thread the three components p of ONE row model (lanes r, r+8, r+16) for two column models, so
 // the nine sums of a pair meet in one thread without any shuffle.
 //
-// Roles: warp 0 = bulk-copy producer (operand planes are stored in HBM as shared-memory images in the
-// canonical K-major core-matrix layout, so tiles arrive by plain 1-D cp.async.bulk), warp 1 = MMA issuer
-// (one thread) and TMEM owner, warps 2..17 = two epilogue teams of 8 warps (4 TMEM quadrants x 2 column
-// halves) that alternate over tiles on two TMEM accumulator buffers of 144 columns; a row tile's A operand is moved
-// once from a shared-memory staging area into TMEM (tcgen05.cp, columns 288...) and read from there by every MMA.
-// The epilogue's sink is a template parameter: packed store (a5), threshold compaction, or row statistics.
+// Roles (20 warps): one service warpgroup -- warp 0 = bulk-copy producer (operand planes are stored in HBM as
+// shared-memory images in the canonical K-major core-matrix layout, so tiles arrive by plain 1-D cp.async.bulk),
+// warp 1 = MMA issuer (one thread) and TMEM owner, warps 2, 3 idle -- that hands most of its registers to the four
+// epilogue warpgroups (setmaxnreg), warps 4..19 = two epilogue teams of 8 warps (4 TMEM quadrants x 2 column halves)
+// that alternate over tiles.  TMEM accumulator buffers of 144 columns: three for L <= 128, two above; a row tile's A
+// operand is moved once from a shared-memory staging area into TMEM (tcgen05.cp, columns after the buffers) and read
+// from there by every MMA (for L in 97..128 the last two slabs of the third digit stay in the staging area, which is
+// then double-buffered).  An epilogue team holds a buffer only while it loads and recombines the three levels; the closed
+// form runs after the buffer has been handed back.  The epilogue's sink is a template parameter: packed store (a5),
+// threshold compaction, or row statistics.
 #pragma once
 #include "common.cuh"
 #include "epilogue.cuh"
@@ -33,13 +37,35 @@
 
 namespace clusco {
 
+__host__ __device__ constexpr int i8_a_stagings(int ks);
 constexpr double I8_KAPPA = 127.0 / 128.0;
 constexpr int I8_MAX_STAGES = 6;               // B stages (whole column tiles) in flight: as many as shared memory holds, up to this
 constexpr int I8_ACC_COLS = 144;               // TMEM columns per accumulator buffer (3 levels x 48)
-constexpr int I8_ACC_BUFS = 2;
-constexpr int I8_A_TMEM_COL = I8_ACC_BUFS * I8_ACC_COLS;   // the A tile lives in TMEM columns 288 .. 288 + 24 ksteps
+constexpr int I8_MAX_ACC_BUFS = 3;
+// accumulator buffers: three where tensor memory holds them beside the A tile (3 x 144 + 24 ksteps <= 512: L <= 96), else two;
+// the A tile lives in the columns after the buffers
+// (k-steps = 4, L in 97..128, gets its third buffer by leaving the A tile's third digit in shared memory: see i8_a_tmem_digits)
+__host__ __device__ constexpr int i8_acc_bufs(int ks) { return ks <= 4 ? 3 : 2; }
+// (k-step, digit) slabs of the A tile kept in tensor memory, in the order digit-major; the remaining ones (the last
+// k-steps of the third digit, if any) are read from the shared-memory staging area by their (narrow, N = 48) MMAs
+__host__ __device__ constexpr int i8_a_tmem_slabs(int ks)
+{
+    return (512 - i8_acc_bufs(ks) * I8_ACC_COLS) / 8 < 3 * ks ? (512 - i8_acc_bufs(ks) * I8_ACC_COLS) / 8 : 3 * ks;
+}
+__host__ __device__ constexpr int i8_a_stagings(int ks) { return i8_a_tmem_slabs(ks) < 3 * ks ? 2 : 1; }
 constexpr int I8_EPI_WARPS = 16;
-constexpr int I8_THREADS = (2 + I8_EPI_WARPS) * 32;
+constexpr int I8_SERVICE_WARPS = 4;            // one warpgroup: bulk-copy producer, MMA issuer, two idle warps
+// (the service warps take the LOWEST warp numbers: measured, waiting service warps with high numbers -- which issue first
+// among a scheduler's ready warps -- cost the epilogue 4-12 % at L <= 96)
+constexpr int I8_PRODUCER_WARP = 0, I8_MMA_WARP = 1;
+constexpr int I8_THREADS = (I8_SERVICE_WARPS + I8_EPI_WARPS) * 32;
+// Register split (setmaxnreg works on warpgroups of four warps and moves registers inside the CTA's own allocation): the
+// kernel starts with 96 registers per thread (five warps per scheduler); the service warpgroup shrinks to
+// I8_REGS_SERVICE, which frees 128 x (96 - 24) registers, and the four epilogue warpgroups grow to I8_REGS_EPI, which
+// takes 512 x (112 - 96) <= that.  (Asking for more than was freed never completes: the increase waits for registers.)
+constexpr int I8_REGS_SERVICE = 24;
+constexpr int I8_REGS_EPI = 112;
+static_assert(I8_EPI_WARPS * (I8_REGS_EPI - 96) <= I8_SERVICE_WARPS * (96 - I8_REGS_SERVICE), "register split must balance");
 constexpr int I8_HIT_CAP = 64;                 // BELOW: hits staged per epilogue warp before one atomic reserves their slots
 constexpr size_t I8_HIT_BYTES = (size_t)I8_EPI_WARPS * I8_HIT_CAP * 12;
 
@@ -52,13 +78,18 @@ static inline bool i8tc_supported(int32_t L) { return L >= 1 && L <= 32 * I8_MAX
 // three passes: FP64 centroid -> max|a| (scale exponent) -> fixed-point integers I.  The integers of a round
 // (4 k-steps = 128 atoms) go through a warp-private shared-memory strip so that each lane can pack the digit
 // bytes of 4 consecutive atoms of one component into one 32-bit store of the operand images.
+// Per-model records the epilogue reads (sum of squares as two floats, scale 2^e), stored per column tile of 16 models as
+// [Thi[16] | Tlo[16] | pw[16]] with model m of the tile at slot i8_col_slot(m) -- the order of the B rows -- so that the
+// two column models of an epilogue thread (c and c + 4) are adjacent: one 8-byte load per quantity.
+constexpr int I8_CSTAT_TILE = 48;
+__host__ __device__ __forceinline__ int i8_col_slot(int m16) { return (m16 & 8) | ((m16 & 3) << 1) | ((m16 >> 2) & 1); }
 constexpr int I8_PREP_WARPS = 8;
 constexpr int I8_PREP_STRIP = 4 * 97;          // ints per warp and round: 4 k-steps x (96 + 1 pad)
 
 __global__ void __launch_bounds__(I8_PREP_WARPS * 32) i8_prep_kernel(const float* __restrict__ coords, int64_t N, int32_t L,
                                                                      int32_t ks, int64_t row_slots, int64_t col_slots,
                                                                      int64_t stat_slots, int8_t* __restrict__ Ap,
-                                                                     int8_t* __restrict__ Bp, PairStat* __restrict__ pstat)
+                                                                     int8_t* __restrict__ Bp, float* __restrict__ cstat)
 {
     __shared__ int strip_s[I8_PREP_WARPS][I8_PREP_STRIP];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
@@ -115,7 +146,7 @@ __global__ void __launch_bounds__(I8_PREP_WARPS * 32) i8_prep_kernel(const float
     // B image: column tile n/16, o = position of this model among the 16 columns of a component block
     const int64_t b_tile = n >> 4;
     const int m16 = (int)(n & 15);
-    const int b_o = (m16 & 8) | ((m16 & 3) << 1) | ((m16 >> 2) & 1);
+    const int b_o = i8_col_slot(m16);
     const int sub = lane >> 3, j = lane & 7;               // packing role: k-step 4 r + sub, atoms 4 j .. 4 j + 3 of it
     const int kc = j >> 2, kb = (j & 3) * 4;
     int* strip = strip_s[wib];
@@ -175,13 +206,13 @@ __global__ void __launch_bounds__(I8_PREP_WARPS * 32) i8_prep_kernel(const float
     finite = __all_sync(0xffffffffu, finite);
     if (lane == 0) {
         const double T = ldexp((double)sumsq, 2 * ex - 46);          // KAPPA^2 sum |a|^2, Angstrom^2
-        PairStat ps;
-        ps.Thi = (float)T;
-        ps.Tlo = (float)(T - (double)ps.Thi);
-        if (!finite || !finite_range) ps.Thi = __int_as_float(0x7fc00000);  // NaN/Inf coordinates poison this model's pairs
-        ps.pw = pow2i(ex);
-        ps.pad = 0.0f;
-        pstat[n] = ps;
+        float Thi = (float)T;
+        const float Tlo = (float)(T - (double)Thi);
+        if (!finite || !finite_range) Thi = __int_as_float(0x7fc00000);     // NaN/Inf coordinates poison this model's pairs
+        float* rec = cstat + b_tile * I8_CSTAT_TILE + b_o;
+        rec[0] = Thi;
+        rec[16] = Tlo;
+        rec[32] = pow2i(ex);
     }
 }
 
@@ -209,7 +240,7 @@ __device__ __forceinline__ void i8_tile_from_linear(const I8Tiles& t, int64_t li
 struct I8Params {
     const int8_t* Ap;
     const int8_t* Bp;
-    const PairStat* pstat;
+    const float* cstat;    // per-model records, I8_CSTAT_TILE floats per column tile (see i8_prep_kernel)
     float* out;
     int64_t N, row_begin, row_end, base;
     int32_t stages;        // B ring depth (one stage = the whole column tile, KS k-steps)
@@ -230,17 +261,25 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     constexpr int ks = KS;
     constexpr uint32_t STAGE_BYTES = KS * I8_B_SLAB;
     const int stages = P.stages;
-    uint8_t* sA = smem;                                          // staging for the next row tile: 3 digits x KS x 4096
-    uint8_t* sB = smem + (size_t)3 * ks * I8_A_SLAB;             // stages x KS x 4608
+    constexpr int NB = i8_acc_bufs(KS);
+    constexpr int AS = i8_a_tmem_slabs(KS);                      // slabs of the A tile resident in tensor memory
+    static_assert(NB * I8_ACC_COLS + 8 * AS <= 512 && AS >= 2 * KS, "tensor memory budget");
+    // A staging: one area when the whole tile moves on into tensor memory, two (used alternately) when some slabs are read
+    // from it for the whole row tile -- so that the next row tile's A still arrives while the current one is in use
+    constexpr int NA = i8_a_stagings(KS);
+    constexpr uint32_t A_BYTES = 3u * KS * I8_A_SLAB;
+    uint8_t* sA = smem;                                          // NA x 3 digits x KS x 4096
+    uint8_t* sB = smem + (size_t)NA * A_BYTES;                   // stages x KS x 4608
     uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)stages * STAGE_BYTES);
-    // barrier map: [0,S) b_full, [S,2S) b_empty, 2S a_full, 2S+1 a_empty, 2S+2.. acc_full[2], acc_empty[2]
+    // barrier map: [0,S) b_full, [S,2S) b_empty, 2S.. a_full[2], a_empty[2], 2S+4.. acc_full[3], acc_empty[3]
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto B_FULL = [&](uint32_t s) { return bar0 + 8u * s; };
     auto B_EMPTY = [&](uint32_t s) { return bar0 + 8u * (stages + s); };
-    const uint32_t A_FULL = bar0 + 8u * (2 * stages), A_EMPTY = A_FULL + 8u;
-    auto ACC_FULL = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 2 + b); };
-    auto ACC_EMPTY = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 2 + I8_ACC_BUFS + b); };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * stages + 2 + 2 * I8_ACC_BUFS);
+    auto A_FULL = [&](uint32_t a) { return bar0 + 8u * (2 * stages + a); };
+    auto A_EMPTY = [&](uint32_t a) { return bar0 + 8u * (2 * stages + 2 + a); };
+    auto ACC_FULL = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 4 + b); };
+    auto ACC_EMPTY = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 4 + I8_MAX_ACC_BUFS + b); };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * stages + 4 + 2 * I8_MAX_ACC_BUFS);
 
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -248,15 +287,17 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             ptx::mbar_init(B_FULL(s), 1);
             ptx::mbar_init(B_EMPTY(s), 1);
         }
-        ptx::mbar_init(A_FULL, 1);
-        ptx::mbar_init(A_EMPTY, 1);
-        for (int b = 0; b < I8_ACC_BUFS; ++b) {
+        for (int a = 0; a < NA; ++a) {
+            ptx::mbar_init(A_FULL(a), 1);
+            ptx::mbar_init(A_EMPTY(a), 1);
+        }
+        for (int b = 0; b < NB; ++b) {
             ptx::mbar_init(ACC_FULL(b), 1);
             ptx::mbar_init(ACC_EMPTY(b), I8_EPI_WARPS / 2);
         }
         ptx::fence_mbar_init();
     }
-    if (warp == 1) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
+    if (warp == I8_MMA_WARP) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
@@ -269,7 +310,9 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     int64_t I0, J0;
     i8_tile_from_linear(P.tiles, t0, I0, J0);
 
-    if (warp == 0) {
+    if (warp < I8_SERVICE_WARPS) {
+    ptx::setmaxnreg_dec<I8_REGS_SERVICE>();
+    if (warp == I8_PRODUCER_WARP) {
         // ===== producer: one elected lane streams operand images with 1-D bulk copies =====
         if (lane == 0) {
             int64_t I = I0, J = J0;
@@ -277,9 +320,10 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             uint32_t a_loads = 0, stage = 0, phase = 0;
             for (uint32_t n = 0; n < ntiles; ++n) {
                 if (I != curI) {
-                    ptx::mbar_wait(A_EMPTY, (a_loads & 1) ^ 1);
-                    ptx::mbar_expect_tx(A_FULL, 3u * ks * I8_A_SLAB);
-                    ptx::bulk_g2s(ptx::smem_u32(sA), P.Ap + (size_t)I * 3 * ks * I8_A_SLAB, 3u * ks * I8_A_SLAB, A_FULL);
+                    const uint32_t a = a_loads % NA;             // load number a_loads / NA of that staging area
+                    ptx::mbar_wait(A_EMPTY(a), ((a_loads / NA) & 1) ^ 1);
+                    ptx::mbar_expect_tx(A_FULL(a), A_BYTES);
+                    ptx::bulk_g2s(ptx::smem_u32(sA + (size_t)a * A_BYTES), P.Ap + (size_t)I * A_BYTES, A_BYTES, A_FULL(a));
                     ++a_loads;
                     curI = I;
                 }
@@ -291,19 +335,20 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 if (++J >= Tc) { ++I; J = 2 * I; }
             }
         }
-    } else if (warp == 1) {
+    } else if (warp == I8_MMA_WARP) {
         // ===== MMA issuer: the whole warp walks the loop (warp-uniform control flow and addresses, so the
         // operands live in uniform registers); one elected lane issues =====
         constexpr uint32_t ID144 = ptx::idesc_s8(128, 144), ID96 = ptx::idesc_s8(128, 96), ID48 = ptx::idesc_s8(128, 48);
         // descriptor = hi word (SBO 256 B, version 1) | lo word (LBO 128 B, start address >> 4)
         constexpr uint64_t DESC_HI = (uint64_t)((256u >> 4) | (1u << 14)) << 32;
-        const uint32_t a_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sA) & 0x3FFFFu) >> 4);
+        uint32_t a_lo0 = 0;                                      // descriptor low word of the current row tile's staging area
         const uint32_t b_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sB) & 0x3FFFFu) >> 4);
-        const uint32_t a_tm = tmem + I8_A_TMEM_COL;              // digit a, k-step k at column 8 (a KS + k)
+        const uint32_t a_tm = tmem + NB * I8_ACC_COLS;           // digit a, k-step k at column 8 (a KS + k)
         uint32_t rem = 0;                                        // tiles left in the current row tile
         uint32_t next_rem = (uint32_t)(Tc - J0);
         uint32_t next_row_len = (uint32_t)(Tc - 2 * (I0 + 1));   // each further row is two tiles shorter
         uint32_t a_uses = 0, stage = 0, phase = 0;
+        uint32_t buf = 0, acc_par = 0;                           // tile n: buffer n % NB, use number n / NB of it
         for (uint32_t n = 0; n < ntiles; ++n) {
             if (rem == 0) {
                 // new row tile: move its A operand from the shared-memory staging area into tensor memory
@@ -311,20 +356,21 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 rem = next_rem;
                 next_rem = next_row_len;
                 next_row_len -= 2;
-                ptx::mbar_wait(A_FULL, a_uses & 1);
+                const uint32_t a = a_uses % NA;
+                ptx::mbar_wait(A_FULL(a), (a_uses / NA) & 1);
                 ptx::tc_fence_after();
+                a_lo0 = ((128u >> 4) << 16) | ((ptx::smem_u32(sA + (size_t)a * A_BYTES) & 0x3FFFFu) >> 4);
                 if (ptx::elect_one()) {
 #pragma unroll
-                    for (int s = 0; s < 3 * KS; ++s)
+                    for (int s = 0; s < AS; ++s)
                         ptx::tmem_cp_128x256b(a_tm + 8 * s, DESC_HI | (a_lo0 + s * (I8_A_SLAB >> 4)));
-                    ptx::tc_commit(A_EMPTY);
+                    if (AS == 3 * KS) ptx::tc_commit(A_EMPTY(a));  // staging area free once the copies are done
                 }
                 __syncwarp();
                 ++a_uses;
             }
             --rem;
-            const uint32_t buf = n & 1;
-            ptx::mbar_wait(ACC_EMPTY(buf), ((n >> 1) & 1) ^ 1);
+            ptx::mbar_wait(ACC_EMPTY(buf), acc_par ^ 1);
             ptx::mbar_wait(B_FULL(stage), phase);
             ptx::tc_fence_after();
             if (ptx::elect_one()) {
@@ -335,17 +381,27 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                     const uint64_t db = DESC_HI | (b_lo + k * (I8_B_SLAB >> 4));
                     ptx::mma_i8_ts(d, a_tm + 8 * k, db, ID144, k > 0);
                     ptx::mma_i8_ts(d + 48, a_tm + 8 * (KS + k), db, ID96, 1);
-                    ptx::mma_i8_ts(d + 96, a_tm + 8 * (2 * KS + k), db, ID48, 1);
+                    if (2 * KS + k < AS)
+                        ptx::mma_i8_ts(d + 96, a_tm + 8 * (2 * KS + k), db, ID48, 1);
+#ifndef I8_SKIP_SS
+                    else
+                        ptx::mma_i8(d + 96, DESC_HI | (a_lo0 + (2 * KS + k) * (I8_A_SLAB >> 4)), db, ID48, 1);
+#endif
                 }
                 ptx::tc_commit(B_EMPTY(stage));
                 ptx::tc_commit(ACC_FULL(buf));
+                // third digit read from the staging area: it is free only after the row tile's last MMA
+                if (AS < 3 * KS && rem == 0) ptx::tc_commit(A_EMPTY((a_uses - 1) % NA));
             }
             __syncwarp();
             if (++stage == (uint32_t)stages) { stage = 0; phase ^= 1; }
+            if (++buf == (uint32_t)NB) { buf = 0; acc_par ^= 1; }
         }
+    }
     } else {
+        ptx::setmaxnreg_inc<I8_REGS_EPI>();
         // ===== epilogue =====
-        const int ew = warp - 2;
+        const int ew = warp - I8_SERVICE_WARPS;
         const int team = ew >> 3, half = (ew & 7) >> 2;          // column half: models 8*half .. 8*half+7 of the tile
         const int quad = warp & 3;                               // TMEM lanes 32 quad .. 32 quad + 31
         const int r = lane >> 2, c4 = lane & 3;
@@ -356,7 +412,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
         int32_t curI = -1, i = 0;
         int64_t rowoff = 0;
         bool row_ok = false;
-        PairStat si = {0.0f, 0.0f, 1.0f, 0.0f};
+        float si_Thi = 0.0f, si_Tlo = 0.0f, si_pw = 1.0f;          // row model's record
         // The closed form of a tile is evaluated in two halves, software-pipelined over the team's tiles: the
         // invariants (c2, c1, det) right after the accumulators are read, the serial root-finding half (Viete,
         // Newton, finish, store) one tile later, between the issue of the next tile's TMEM loads and their
@@ -468,27 +524,52 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 }
             }
         };
-        auto tile_body = [&](const uint32_t n, Pending& pend, const Pending& prev, const bool have_prev) {
+        uint32_t buf = (uint32_t)team, acc_par = 0;             // this team's tile n: buffer n % NB, use number n / NB of it
+        auto tile_body = [&](Pending& pend, const Pending& prev, const bool have_prev) {
             if (I != curI) {                                     // per-row quantities (warp-uniform branch)
                 curI = I;
                 i = I * I8_ROW_MODELS + quad * 8 + r;
                 row_ok = i < N32 && i >= (int32_t)P.row_begin && i < (int32_t)P.row_end;
-                si = P.pstat[i];                                 // slots beyond N hold neutral records
+                const float* ri = P.cstat + (size_t)(i >> 4) * I8_CSTAT_TILE + i8_col_slot(i & 15);   // slots beyond N hold neutral records
+                // (the identity shuffles make the warp wait for these three loads HERE, in the rare row-change path: left
+                // pending, their scoreboard slot is shared with the per-tile loads below and the first read of si_* in
+                // every later tile then waits for those -- measured: 6 % of the epilogue's stall samples at L = 100)
+                si_Thi = __shfl_sync(0xffffffffu, ri[0], lane);
+                si_Tlo = __shfl_sync(0xffffffffu, ri[16], lane);
+                si_pw = __shfl_sync(0xffffffffu, ri[32], lane);
                 rowoff = (int64_t)i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
             }
-            // per-model records of this thread's two column models, requested before the accumulator wait
             const int32_t j0 = J * I8_COL_MODELS + half * 8 + c4;
-            const PairStat sj0 = P.pstat[j0], sj1 = P.pstat[j0 + 4];
-            const uint32_t buf = (uint32_t)team;                 // tile n uses accumulator n & 1 = team
-            ptx::mbar_wait(ACC_FULL(buf), (n >> 1) & 1);
+            // records of this thread's two column models: three 8-byte loads that land directly in the register pairs
+            // the packed arithmetic reads (no moves, so nothing waits for them before the tile's finish, one tile later)
+            {
+                const float* cj = P.cstat + (size_t)J * I8_CSTAT_TILE + half * 8 + c4 * 2;
+                pend.Thj = *reinterpret_cast<const float2*>(cj);
+                pend.Tlj = *reinterpret_cast<const float2*>(cj + 16);
+                pend.pwj = *reinterpret_cast<const float2*>(cj + 32);
+            }
+            pend.Thi = si_Thi; pend.Tlo = si_Tlo; pend.pw = si_pw;
+            pend.dst = P.out + rowoff + j0;
+            pend.i = i;
+            pend.j0 = j0;
+            pend.ok0 = row_ok && j0 < N32 && j0 > i;             // masked pairs are simply not stored
+            pend.ok1 = row_ok && j0 + 4 < N32 && j0 + 4 > i;
+            // advance to the team's next tile (two tiles on)
+#pragma unroll
+            for (int s = 0; s < 2; ++s)
+                if (++J >= Tc32) { ++I; J = 2 * I; }
+            ptx::mbar_wait(ACC_FULL(buf), acc_par);
             ptx::tc_fence_after();
             const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16) + buf * I8_ACC_COLS + half * 8;
             // m[3p+q] = (.x, .y): pairs (row model r, column model c4 + 8 half) and (.., + 4); Gram sums in units
             // of 2^46.  The two pairs of a thread go through the closed form together, on packed fp32 arithmetic.
+            // The accumulator buffer is held only for the loads and the level recombination below and handed back
+            // to the MMA warp before any of the closed form runs (at L <= 128 the epilogue, not the tensor pipe, sets the
+            // pace: every cycle the buffer is held is a cycle the next tile's MMAs cannot start).
             float2 m[9];
             {
                 // levels 1 and 2 first: T = 2^8 V1 + V2 fits int32 (|T| < 2^31 for L <= 256 because |d0| <= 127)
-                uint32_t v1[3][2][4], v2[3][2][4];
+                uint32_t v1[3][2][4], v2[3][2][4], v0[3][2][4];
 #pragma unroll
                 for (int q = 0; q < 3; ++q)
 #pragma unroll
@@ -496,8 +577,12 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                         ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 48 + 16 * q, v1[q][h]);
                         ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 96 + 16 * q, v2[q][h]);
                     }
-                if (have_prev) finish_pending(prev);             // previous tile's serial half, under the load latency
                 ptx::tmem_ld_wait();
+                // level 0 is requested before levels 1 and 2 are converted, so its latency is covered by that work
+#pragma unroll
+                for (int q = 0; q < 3; ++q)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 16 * q, v0[q][h]);
                 const float2 s30 = make_float2(0x1p-30f, 0x1p-30f);
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
@@ -507,14 +592,13 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                     m[3 + q] = __fmul2_rn(make_float2(T(0, 2), T(0, 3)), s30);
                     m[6 + q] = __fmul2_rn(make_float2(T(1, 0), T(1, 1)), s30);
                 }
-            }
-            {
-                uint32_t v0[3][2][4];
-#pragma unroll
-                for (int q = 0; q < 3; ++q)
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 16 * q, v0[q][h]);
                 ptx::tmem_ld_wait();
+                // the accumulator buffer is free again
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
+                buf += 2;                                        // the team's next tile is two tiles on
+                if (buf >= (uint32_t)NB) { buf -= NB; acc_par ^= 1; }
                 const float2 s14 = make_float2(0x1p-14f, 0x1p-14f);
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
@@ -524,33 +608,17 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                     m[6 + q] = __ffma2_rn(make_float2(F(1, 0), F(1, 1)), s14, m[6 + q]);
                 }
             }
-            // the accumulator buffer is free again
-            ptx::tc_fence_before();
-            __syncwarp();
-            if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
-
+            // two independent chains: this tile's invariants and the previous tile's serial root-finding half
+            if (have_prev) finish_pending(prev);
             pend.inv = eq2_invariants(m);
-            pend.Thi = si.Thi; pend.Tlo = si.Tlo; pend.pw = si.pw;
-            pend.Thj = make_float2(sj0.Thi, sj1.Thi);
-            pend.Tlj = make_float2(sj0.Tlo, sj1.Tlo);
-            pend.pwj = make_float2(sj0.pw, sj1.pw);
-            pend.dst = P.out + rowoff + j0;
-            pend.i = i;
-            pend.j0 = j0;
-            pend.ok0 = row_ok && j0 < N32 && j0 > i;             // masked pairs are simply not stored
-            pend.ok1 = row_ok && j0 + 4 < N32 && j0 + 4 > i;
-            // advance two tiles
-#pragma unroll
-            for (int s = 0; s < 2; ++s)
-                if (++J >= Tc32) { ++I; J = 2 * I; }
         };
         bool last_is_A = true;
         for (uint32_t n = team; n < ntiles; n += 4) {
-            tile_body(n, pendA, pendB, have_pend);
+            tile_body(pendA, pendB, have_pend);
             have_pend = true;
             last_is_A = true;
             if (n + 2 >= ntiles) break;
-            tile_body(n + 2, pendB, pendA, true);
+            tile_body(pendB, pendA, true);
             last_is_A = false;
         }
         if (have_pend) {
@@ -561,12 +629,13 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     }
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 1) ptx::tmem_dealloc(tmem, 512);
+    if (warp == I8_MMA_WARP) ptx::tmem_dealloc(tmem, 512);
 }
 
 static inline size_t i8tc_smem_bytes(int ks, int stages)
 {
-    return (size_t)3 * ks * I8_A_SLAB + (size_t)stages * ks * I8_B_SLAB + 8 * (2 * stages + 2 + 2 * I8_ACC_BUFS) + 16;
+    return (size_t)i8_a_stagings(ks) * 3 * ks * I8_A_SLAB + (size_t)stages * ks * I8_B_SLAB +
+           8 * (2 * stages + 4 + 2 * I8_MAX_ACC_BUFS) + 16;
 }
 static inline int i8tc_stages(int ks, size_t extra)
 {
@@ -582,7 +651,7 @@ static inline int i8tc_prepare(const float* coords, int64_t N, int32_t L, const 
     const int64_t row_slots = w.row_tiles * I8_ROW_MODELS, col_slots = w.col_tiles * I8_COL_MODELS;
     i8_prep_kernel<<<(unsigned)((w.Np + I8_PREP_WARPS - 1) / I8_PREP_WARPS), I8_PREP_WARPS * 32, 0, s>>>(
         coords, N, L, ks, row_slots, col_slots, w.Np, (int8_t*)(ws + w.off_i8a), (int8_t*)(ws + w.off_i8b),
-        (PairStat*)(ws + w.off_pstat));
+        (float*)(ws + w.off_pstat));
     CLUSCO_CUDA_TRY(cudaGetLastError());
     return CLUSCO_OK;
 }
@@ -595,7 +664,7 @@ static inline int i8tc_compute(int64_t N, int32_t L, int64_t row_begin, int64_t 
     I8Params P;
     P.Ap = (const int8_t*)(ws + w.off_i8a);
     P.Bp = (const int8_t*)(ws + w.off_i8b);
-    P.pstat = (const PairStat*)(ws + w.off_pstat);
+    P.cstat = (const float*)(ws + w.off_pstat);
     P.out = out;
     P.sink = sink;
     P.N = N;
