@@ -138,36 +138,39 @@ __device__ __forceinline__ EPairT<V> eq2_energy(const EqInvariants<V> inv)
     const V c2 = inv.c2, c1 = inv.c1, d = inv.d;
     // largest root of the cubic, Viete:  l1 = q + 2 sqrt(p) cos(acos(rr / p^1.5) / 3)
     // with q = c2 / 3:  p = (c2^2 - 3 c1) / 9 = q^2 - c1 / 3,   r = (27 d^2 + c2 (2 c2^2 - 9 c1)) / 54 = d^2 / 2 + q (q^2 - c1 / 2)
+    // p is kept away from zero (three equal roots, or M == 0) by a floor far below anything that matters; 1 / sqrt(p)
+    // then serves both sqrt(p) and p^-1.5.  Where p sits on the floor the ratio may overflow or be 0 * inf: the saturating
+    // FMA inside cos_third_acos maps +-inf to 0 / 1 and NaN to 0, and the factor sqrt(p) ~ 1e-15 makes the term vanish.
     const V q = mul(c2, splat<V>(1.0f / 3.0f));
-    V pp = fma(q, q, mul(c1, splat<V>(-1.0f / 3.0f)));
-    pp = map(pp, [](float t) { return t > 0.0f ? t : 0.0f; });
+    const V qq = mul(q, q);
+    const V pp = map(fma(c1, splat<V>(-1.0f / 3.0f), qq), [](float t) { return fmaxf(t, 1e-30f); });
+    const V isp = map(pp, [](float t) { return rsqrt_fast(t); });
+    const V sp = mul(pp, isp);
     const V d2 = mul(d, d);
-    const V rr = fma(q, fma(q, q, mul(c1, splat<V>(-0.5f))), mul(d2, splat<V>(0.5f)));
-    const V sp = map(pp, [](float t) { return sqrt_fast(t); });
-    const V ps = mul(pp, sp);
-    const V ratio = zip3(pp, rr, ps, [](float p_, float r_, float ps_) { return p_ > 0.0f ? r_ * rcp_fast(ps_) : 1.0f; });
-    V l1 = fma(mul(splat<V>(2.0f), sp), cos_third_acos(ratio), q);    // cos(theta / 3), theta = acos(ratio) in [0, pi]
+    const V rr = fma(q, fma(c1, splat<V>(-0.5f), qq), mul(d2, splat<V>(0.5f)));
+    const V ratio = mul(rr, mul(mul(isp, isp), isp));
+    V l1 = fma(add(sp, sp), cos_third_acos(ratio), q);               // cos(theta / 3), theta = acos(ratio) in [0, pi]
     l1 = zip(l1, q, [](float a_, float b_) { return fmaxf(a_, b_); }); // l1 >= trace/3 always
     const V is1 = map(l1, [](float t) { return rsqrt_fast(t); });
     const V s1 = mul(l1, is1);
     const V inv1 = mul(is1, is1);
     // deflation: (s2 + S s3)^2 = (c1 - d^2/l1)/l1 + 2 d / s1
-    const V w2 = fma(mul(splat<V>(2.0f), d), is1, mul(fma(neg(d2), inv1, c1), inv1));
-    const V w = map(w2, [](float t) { return sqrt_fast(t > 0.0f ? t : 0.0f); });
+    const V w2 = fma(add(d, d), is1, mul(fma(neg(d2), inv1, c1), inv1));
+    const V w = map(w2, [](float t) { return sqrt_fast(fmaxf(t, 0.0f)); });
     const V E0 = add(s1, w);
 
     // one Newton step on the quartic; skipped where f' is tiny against E^3 (s2 + S s3 -> 0: the
     // quartic's roots pair up and the deflated value above is the well-conditioned one)
     const V t = fma(E0, E0, neg(c2));
-    const V f = fma(t, t, fma(mul(splat<V>(-8.0f), d), E0, mul(splat<V>(-4.0f), c1)));
-    const V fp = fma(mul(splat<V>(4.0f), E0), t, mul(splat<V>(-8.0f), d));
-    const V lim = mul(mul(splat<V>(1e-3f), E0), mul(E0, E0));
-    // M == 0 (L = 1, or every atom on the centroid): E = 0 (the lines above then hold 0 * inf, selected away
-    // here, so the function stays branch-free); a NaN in M gives c2 = NaN and passes through as NaN
+    const V d8 = mul(d, splat<V>(-8.0f));
+    const V f = fma(t, t, fma(d8, E0, mul(c1, splat<V>(-4.0f))));
+    const V fp = fma(mul(E0, splat<V>(4.0f)), t, d8);
+    const V lim = mul(mul(E0, splat<V>(1e-3f)), mul(E0, E0));
+    // M == 0 (L = 1, or every atom on the centroid): the floor above gives E0 ~ 3e-8 in units where |M| <= 2^8, i.e. below
+    // 1e-5 A^2 in c^2 and clamped away where both models are points; a NaN in M gives q = NaN and passes through as NaN
     EPairT<V> r;
-    r.E0 = zip(c2, E0, [](float c2_, float e_) { return c2_ > 1e-30f ? e_ : c2_ * 0.0f; });
-    const V step = zip3(f, fp, lim, [](float f_, float fp_, float lim_) { return fp_ > lim_ ? f_ * rcp_fast(fp_) : 0.0f; });
-    r.delta = zip(c2, step, [](float c2_, float s_) { return c2_ > 1e-30f ? s_ : 0.0f; });
+    r.E0 = E0;
+    r.delta = zip3(f, fp, lim, [](float f_, float fp_, float lim_) { return fp_ > lim_ ? f_ * rcp_fast(fp_) : 0.0f; });
     return r;
 }
 
