@@ -22,13 +22,13 @@
 // Roles (20 warps): one service warpgroup -- warp 0 = bulk-copy producer (operand planes are stored in HBM as
 // shared-memory images in the canonical K-major core-matrix layout, so tiles arrive by plain 1-D cp.async.bulk),
 // warp 1 = MMA issuer (one thread) and TMEM owner, warps 2, 3 idle -- that hands most of its registers to the four
-// epilogue warpgroups (setmaxnreg), warps 4..19 = two epilogue teams of 8 warps (4 TMEM quadrants x 2 column halves)
-// that alternate over tiles.  TMEM accumulator buffers of 144 columns: three for L <= 128, two above; a row tile's A
-// operand is moved once from a shared-memory staging area into TMEM (tcgen05.cp, columns after the buffers) and read
-// from there by every MMA (for L in 97..128 the last two slabs of the third digit stay in the staging area, which is
-// then double-buffered).  An epilogue team holds a buffer only while it loads and recombines the three levels; the closed
-// form runs after the buffer has been handed back.  The epilogue's sink is a template parameter: packed store (a5),
-// threshold compaction, or row statistics.
+// epilogue warpgroups (setmaxnreg); warps 4..19 = four epilogue teams of 4 warps (one per TMEM quadrant) that take the
+// tiles in turn, each thread carrying four pairs of a tile (two packed groups, two independent dependency chains).
+// TMEM accumulator buffers of 144 columns: three for L <= 160, two above; a row tile's A operand is moved once from a
+// shared-memory staging area into TMEM (tcgen05.cp, columns after the buffers) and read from there by every MMA (for L in
+// 97..160 some slabs of the third digit stay in the staging area, which is then double-buffered).  A team holds a
+// buffer only while it loads and recombines the three levels; the closed form runs after the buffer has been handed
+// back.  The epilogue's sink is a template parameter: packed store (a5), threshold compaction, or row statistics.
 #pragma once
 #include "common.cuh"
 #include "epilogue.cuh"
@@ -42,10 +42,13 @@ constexpr double I8_KAPPA = 127.0 / 128.0;
 constexpr int I8_MAX_STAGES = 6;               // B stages (whole column tiles) in flight: as many as shared memory holds, up to this
 constexpr int I8_ACC_COLS = 144;               // TMEM columns per accumulator buffer (3 levels x 48)
 constexpr int I8_MAX_ACC_BUFS = 3;
-// accumulator buffers: three where tensor memory holds them beside the A tile (3 x 144 + 24 ksteps <= 512: L <= 96), else two;
-// the A tile lives in the columns after the buffers
-// (k-steps = 4, L in 97..128, gets its third buffer by leaving the A tile's third digit in shared memory: see i8_a_tmem_digits)
-__host__ __device__ constexpr int i8_acc_bufs(int ks) { return ks <= 4 ? 3 : 2; }
+// Accumulator buffers: three for L <= 160 (k-steps <= 5), two above.  With four epilogue teams of four warps a buffer is
+// held twice as long as with two teams of eight, and two buffers then starve the tensor pipe (measured at L = 100:
+// 3.38 ms with two buffers, 3.05 ms with three); three buffers fit beside the whole A tile for k-steps <= 3, and for
+// k-steps 4 and 5 when 2 respectively 5 slabs of the A tile's third digit stay in shared memory (i8_a_tmem_slabs).
+// k-steps 6..8 keep two buffers: 1-3 % slower than the two-team kernel it replaces at L = 161..224, equal at L = 250.
+constexpr int I8_NB3_MAX_KS = 5;
+__host__ __device__ constexpr int i8_acc_bufs(int ks) { return ks <= I8_NB3_MAX_KS ? 3 : 2; }
 // (k-step, digit) slabs of the A tile kept in tensor memory, in the order digit-major; the remaining ones (the last
 // k-steps of the third digit, if any) are read from the shared-memory staging area by their (narrow, N = 48) MMAs
 __host__ __device__ constexpr int i8_a_tmem_slabs(int ks)
@@ -54,6 +57,7 @@ __host__ __device__ constexpr int i8_a_tmem_slabs(int ks)
 }
 __host__ __device__ constexpr int i8_a_stagings(int ks) { return i8_a_tmem_slabs(ks) < 3 * ks ? 2 : 1; }
 constexpr int I8_EPI_WARPS = 16;
+constexpr int I8_EPI_TEAMS = 4;                // teams of four warps (one per TMEM quadrant) that take the tiles in turn
 constexpr int I8_SERVICE_WARPS = 4;            // one warpgroup: bulk-copy producer, MMA issuer, two idle warps
 // (the service warps take the LOWEST warp numbers: measured, waiting service warps with high numbers -- which issue first
 // among a scheduler's ready warps -- cost the epilogue 4-12 % at L <= 96)
@@ -83,6 +87,7 @@ static inline bool i8tc_supported(int32_t L) { return L >= 1 && L <= 32 * I8_MAX
 // two column models of an epilogue thread (c and c + 4) are adjacent: one 8-byte load per quantity.
 constexpr int I8_CSTAT_TILE = 48;
 __host__ __device__ __forceinline__ int i8_col_slot(int m16) { return (m16 & 8) | ((m16 & 3) << 1) | ((m16 >> 2) & 1); }
+__host__ __device__ __forceinline__ int i8_stat_slot(int m16) { return ((m16 & 3) << 2) | ((m16 >> 2) & 3); }
 constexpr int I8_PREP_WARPS = 8;
 constexpr int I8_PREP_STRIP = 4 * 97;          // ints per warp and round: 4 k-steps x (96 + 1 pad)
 
@@ -209,7 +214,7 @@ __global__ void __launch_bounds__(I8_PREP_WARPS * 32) i8_prep_kernel(const float
         float Thi = (float)T;
         const float Tlo = (float)(T - (double)Thi);
         if (!finite || !finite_range) Thi = __int_as_float(0x7fc00000);     // NaN/Inf coordinates poison this model's pairs
-        float* rec = cstat + b_tile * I8_CSTAT_TILE + b_o;
+        float* rec = cstat + b_tile * I8_CSTAT_TILE + i8_stat_slot(m16);
         rec[0] = Thi;
         rec[16] = Tlo;
         rec[32] = pow2i(ex);
@@ -271,15 +276,17 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     uint8_t* sA = smem;                                          // NA x 3 digits x KS x 4096
     uint8_t* sB = smem + (size_t)NA * A_BYTES;                   // stages x KS x 4608
     uint64_t* bars = reinterpret_cast<uint64_t*>(sB + (size_t)stages * STAGE_BYTES);
-    // barrier map: [0,S) b_full, [S,2S) b_empty, 2S.. a_full[2], a_empty[2], 2S+4.. acc_full[3], acc_empty[3]
+    // barrier map: [0,S) b_full, [S,2S) b_empty, 2S.. a_full[2], a_empty[2], 2S+4.. acc_full[4] (one per epilogue TEAM: a
+    // waiter must see every phase of its barrier, and a team meets a given buffer only every second or third use),
+    // 2S+8.. acc_empty[3] (one per buffer; the MMA warp sees every phase)
     const uint32_t bar0 = ptx::smem_u32(bars);
     auto B_FULL = [&](uint32_t s) { return bar0 + 8u * s; };
     auto B_EMPTY = [&](uint32_t s) { return bar0 + 8u * (stages + s); };
     auto A_FULL = [&](uint32_t a) { return bar0 + 8u * (2 * stages + a); };
     auto A_EMPTY = [&](uint32_t a) { return bar0 + 8u * (2 * stages + 2 + a); };
-    auto ACC_FULL = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 4 + b); };
-    auto ACC_EMPTY = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 4 + I8_MAX_ACC_BUFS + b); };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * stages + 4 + 2 * I8_MAX_ACC_BUFS);
+    auto ACC_FULL = [&](uint32_t t) { return bar0 + 8u * (2 * stages + 4 + t); };
+    auto ACC_EMPTY = [&](uint32_t b) { return bar0 + 8u * (2 * stages + 4 + I8_EPI_TEAMS + b); };
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * stages + 4 + I8_EPI_TEAMS + I8_MAX_ACC_BUFS);
 
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     if (threadIdx.x == 0) {
@@ -291,10 +298,8 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
             ptx::mbar_init(A_FULL(a), 1);
             ptx::mbar_init(A_EMPTY(a), 1);
         }
-        for (int b = 0; b < NB; ++b) {
-            ptx::mbar_init(ACC_FULL(b), 1);
-            ptx::mbar_init(ACC_EMPTY(b), I8_EPI_WARPS / 2);
-        }
+        for (int t = 0; t < I8_EPI_TEAMS; ++t) ptx::mbar_init(ACC_FULL(t), 1);
+        for (int b = 0; b < NB; ++b) ptx::mbar_init(ACC_EMPTY(b), I8_EPI_WARPS / I8_EPI_TEAMS);
         ptx::fence_mbar_init();
     }
     if (warp == I8_MMA_WARP) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
@@ -383,13 +388,11 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                     ptx::mma_i8_ts(d + 48, a_tm + 8 * (KS + k), db, ID96, 1);
                     if (2 * KS + k < AS)
                         ptx::mma_i8_ts(d + 96, a_tm + 8 * (2 * KS + k), db, ID48, 1);
-#ifndef I8_SKIP_SS
                     else
                         ptx::mma_i8(d + 96, DESC_HI | (a_lo0 + (2 * KS + k) * (I8_A_SLAB >> 4)), db, ID48, 1);
-#endif
                 }
                 ptx::tc_commit(B_EMPTY(stage));
-                ptx::tc_commit(ACC_FULL(buf));
+                ptx::tc_commit(ACC_FULL(n % I8_EPI_TEAMS));
                 // third digit read from the staging area: it is free only after the row tile's last MMA
                 if (AS < 3 * KS && rem == 0) ptx::tc_commit(A_EMPTY((a_uses - 1) % NA));
             }
@@ -401,34 +404,23 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
     } else {
         ptx::setmaxnreg_inc<I8_REGS_EPI>();
         // ===== epilogue =====
+        // Four teams of four warps (one per TMEM quadrant) take the tiles in turn.  A thread owns FOUR pairs of a tile: row
+        // model r of its quadrant against column models c, c + 4 (column half 0) and c + 8, c + 12 (half 1) -- two packed
+        // (float2) groups that go through the closed form as two independent dependency chains, and that share the
+        // per-tile bookkeeping (barrier, tile walk, addresses) and the TMEM loads (16x256b.x2 spans both halves).
         const int ew = warp - I8_SERVICE_WARPS;
-        const int team = ew >> 3, half = (ew & 7) >> 2;          // column half: models 8*half .. 8*half+7 of the tile
+        const int team = ew >> 2;                                // 0 .. I8_EPI_TEAMS - 1
         const int quad = warp & 3;                               // TMEM lanes 32 quad .. 32 quad + 31
         const int r = lane >> 2, c4 = lane & 3;
         // tile coordinates and model indices fit 32 bits (N <= 2^24); only the packed offset needs 64
         const int32_t Tc32 = (int32_t)Tc, N32 = (int32_t)P.N;
         int32_t I = (int32_t)I0, J = (int32_t)J0;
-        if (team == 1 && ++J >= Tc32) { ++I; J = 2 * I; }
+        for (int s = 0; s < team; ++s)
+            if (++J >= Tc32) { ++I; J = 2 * I; }
         int32_t curI = -1, i = 0;
         int64_t rowoff = 0;
         bool row_ok = false;
         float si_Thi = 0.0f, si_Tlo = 0.0f, si_pw = 1.0f;          // row model's record
-        // The closed form of a tile is evaluated in two halves, software-pipelined over the team's tiles: the
-        // invariants (c2, c1, det) right after the accumulators are read, the serial root-finding half (Viete,
-        // Newton, finish, store) one tile later, between the issue of the next tile's TMEM loads and their
-        // completion -- two independent dependency chains per thread instead of one.
-        struct Pending {
-            EqInvariants<float2> inv;
-            float Thi, Tlo, pw;                  // row model
-            float2 Thj, Tlj, pwj;                // the two column models
-            float* dst;                          // out + rowoff + j0
-            int32_t i, j0;                       // the pairs are (i, j0) and (i, j0 + 4)
-            bool ok0, ok1;
-        };
-        // two records used alternately (the loop below is unrolled by two tiles), so that handing a tile's invariants
-        // to the next iteration costs no register moves
-        Pending pendA = {}, pendB = {};
-        bool have_pend = false;
         // ROWSTATS: running sum / count of the row this lane group is on (rows persist over consecutive tiles)
         double acc_sum = 0.0;
         int32_t acc_cnt = 0, acc_i = -1;
@@ -462,45 +454,145 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 if (acc_cnt) atomicAdd(P.sink.below + acc_i, acc_cnt);
             }
         };
-        auto finish_pending = [&](const Pending& pend) {
-            const float2 c = eq2_finish(eq2_energy(pend.inv), make_float2(pend.Thi, pend.Thi),
-                                        make_float2(pend.Tlo, pend.Tlo), make_float2(pend.pw, pend.pw), pend.Thj,
-                                        pend.Tlj, pend.pwj, P.invLk);
+        uint32_t buf = (uint32_t)team % NB, full_par = 0;       // this team's tile n: buffer n % NB; visit n / 4 of the team
+        for (uint32_t n = team; n < ntiles; n += I8_EPI_TEAMS) {
+            if (I != curI) {                                     // per-row quantities (warp-uniform branch)
+                curI = I;
+                i = I * I8_ROW_MODELS + quad * 8 + r;
+                row_ok = i < N32 && i >= (int32_t)P.row_begin && i < (int32_t)P.row_end;
+                const float* ri = P.cstat + (size_t)(i >> 4) * I8_CSTAT_TILE + i8_stat_slot(i & 15);   // slots beyond N hold neutral records
+                // (the identity shuffles make the warp wait for these three loads HERE, in the rare row-change path: left
+                // pending, their scoreboard slot is shared with the per-tile loads below and the first read of si_* in
+                // every later tile then waits for those)
+                si_Thi = __shfl_sync(0xffffffffu, ri[0], lane);
+                si_Tlo = __shfl_sync(0xffffffffu, ri[16], lane);
+                si_pw = __shfl_sync(0xffffffffu, ri[32], lane);
+                rowoff = (int64_t)i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
+            }
+            const int32_t j0 = J * I8_COL_MODELS + c4;           // this thread's column models: j0, j0 + 4, j0 + 8, j0 + 12
+            // their records: one 16-byte load per quantity, in the order (j0, j0 + 4 | j0 + 8, j0 + 12) of the two groups;
+            // first used in the last line of eq. 2, a whole closed form away
+            const float* cj = P.cstat + (size_t)J * I8_CSTAT_TILE + c4 * 4;
+            const float4 Thj = *reinterpret_cast<const float4*>(cj);
+            const float4 Tlj = *reinterpret_cast<const float4*>(cj + 16);
+            const float4 pwj = *reinterpret_cast<const float4*>(cj + 32);
+            float* const dst = P.out + rowoff + j0;
+            bool ok[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) ok[e] = row_ok && j0 + 4 * e < N32 && j0 + 4 * e > i;   // masked pairs are not stored
+            const int32_t i_cur = i;
+            // advance to the team's next tile (four tiles on)
+#pragma unroll
+            for (int s = 0; s < 4; ++s)
+                if (++J >= Tc32) { ++I; J = 2 * I; }
+
+            ptx::mbar_wait(ACC_FULL(team), full_par);
+            full_par ^= 1;
+            ptx::tc_fence_after();
+            const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16) + buf * I8_ACC_COLS;
+            // m[g][3p+q] = (.x, .y): pairs (row model r, column models c4 + 8 g and c4 + 8 g + 4); Gram sums in units of
+            // 2^46.  The accumulator buffer is held only for the loads and the level recombination and handed back to the
+            // MMA warp before any of the closed form runs (at L <= 128 the epilogue, not the tensor pipe, sets the pace).
+            float2 m[2][9];
+            {
+                const float2 s30 = make_float2(0x1p-30f, 0x1p-30f), s14 = make_float2(0x1p-14f, 0x1p-14f);
+                // register slots of a 16x256b.x2 load: [0,1] = lane r, half 0; [2,3] = lane r + 8, half 0; [4..7] the same
+                // for half 1; lane window h = 0: p = 0 (lane r), p = 1 (lane r + 8); h = 1: p = 2 (lane r + 16), zero rows
+                uint32_t v1[2][8], v2[2][8], v0[2][8];
+#pragma unroll
+                for (int q = 0; q < 3; ++q) {
+                    // levels 1 and 2 first: T = 2^8 V1 + V2 fits int32 (|T| < 2^31 for L <= 256 because |d0| <= 127)
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        ptx::tmem_ld_16x256b_x2(ta + ((uint32_t)(16 * h) << 16) + 48 + 16 * q, v1[h]);
+                        ptx::tmem_ld_16x256b_x2(ta + ((uint32_t)(16 * h) << 16) + 96 + 16 * q, v2[h]);
+                    }
+                    ptx::tmem_ld_wait();
+                    // level 0 is requested before levels 1 and 2 are converted, so its latency is covered by that work
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) ptx::tmem_ld_16x256b_x2(ta + ((uint32_t)(16 * h) << 16) + 16 * q, v0[h]);
+                    auto T = [&](int h, int e) { return (float)(((int32_t)v1[h][e] << 8) + (int32_t)v2[h][e]); };
+#pragma unroll
+                    for (int g = 0; g < 2; ++g) {
+                        m[g][0 + q] = __fmul2_rn(make_float2(T(0, 4 * g + 0), T(0, 4 * g + 1)), s30);
+                        m[g][3 + q] = __fmul2_rn(make_float2(T(0, 4 * g + 2), T(0, 4 * g + 3)), s30);
+                        m[g][6 + q] = __fmul2_rn(make_float2(T(1, 4 * g + 0), T(1, 4 * g + 1)), s30);
+                    }
+                    ptx::tmem_ld_wait();
+                    auto F = [&](int h, int e) { return (float)(int32_t)v0[h][e]; };
+#pragma unroll
+                    for (int g = 0; g < 2; ++g) {
+                        m[g][0 + q] = __ffma2_rn(make_float2(F(0, 4 * g + 0), F(0, 4 * g + 1)), s14, m[g][0 + q]);
+                        m[g][3 + q] = __ffma2_rn(make_float2(F(0, 4 * g + 2), F(0, 4 * g + 3)), s14, m[g][3 + q]);
+                        m[g][6 + q] = __ffma2_rn(make_float2(F(1, 4 * g + 0), F(1, 4 * g + 1)), s14, m[g][6 + q]);
+                    }
+                }
+                // the accumulator buffer is free again
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
+                buf += I8_EPI_TEAMS % NB;                        // the team's next tile is four tiles on
+                if (buf >= (uint32_t)NB) buf -= NB;
+            }
+            // the closed form, two independent chains (one per group of two pairs)
+            float c[4];
+            {
+                const float2 Ti = make_float2(si_Thi, si_Thi), Tli = make_float2(si_Tlo, si_Tlo), pwi = make_float2(si_pw, si_pw);
+                const EqInvariants<float2> inv0 = eq2_invariants(m[0]), inv1 = eq2_invariants(m[1]);
+                const float2 c01 = eq2_finish(eq2_energy(inv0), Ti, Tli, pwi, make_float2(Thj.x, Thj.y),
+                                              make_float2(Tlj.x, Tlj.y), make_float2(pwj.x, pwj.y), P.invLk);
+                const float2 c23 = eq2_finish(eq2_energy(inv1), Ti, Tli, pwi, make_float2(Thj.z, Thj.w),
+                                              make_float2(Tlj.z, Tlj.w), make_float2(pwj.z, pwj.w), P.invLk);
+                c[0] = c01.x; c[1] = c01.y; c[2] = c23.x; c[3] = c23.y;
+            }
             if (MODE == SINK_STORE) {
-                if (pend.ok0) pend.dst[0] = c.x;
-                if (pend.ok1) pend.dst[4] = c.y;
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+                    if (ok[e]) dst[4 * e] = c[e];
             } else if (MODE == SINK_BELOW) {
-                const bool h0 = pend.ok0 && c.x < P.sink.cutoff, h1 = pend.ok1 && c.y < P.sink.cutoff;
-                const uint32_t m0 = __ballot_sync(0xffffffffu, h0), m1 = __ballot_sync(0xffffffffu, h1);
-                const int add = __popc(m0) + __popc(m1);
-                if (add) {
-                    if (nhit + add > I8_HIT_CAP) flush_hits();
-                    const uint32_t lt = (1u << lane) - 1u;
-                    if (h0) {
-                        const int e = nhit + __popc(m0 & lt);
-                        hit_i[e] = pend.i; hit_j[e] = pend.j0; hit_c[e] = c.x;
+                // two batches of at most 64 candidates (one per group), so that I8_HIT_CAP = 64 slots always suffice
+#pragma unroll
+                for (int g = 0; g < 2; ++g) {
+                    const bool h0 = ok[2 * g] && c[2 * g] < P.sink.cutoff, h1 = ok[2 * g + 1] && c[2 * g + 1] < P.sink.cutoff;
+                    const uint32_t m0 = __ballot_sync(0xffffffffu, h0), m1 = __ballot_sync(0xffffffffu, h1);
+                    const int add = __popc(m0) + __popc(m1);
+                    if (add) {
+                        if (nhit + add > I8_HIT_CAP) flush_hits();
+                        const uint32_t lt = (1u << lane) - 1u;
+                        if (h0) {
+                            const int k = nhit + __popc(m0 & lt);
+                            hit_i[k] = i_cur; hit_j[k] = j0 + 8 * g; hit_c[k] = c[2 * g];
+                        }
+                        if (h1) {
+                            const int k = nhit + __popc(m0) + __popc(m1 & lt);
+                            hit_i[k] = i_cur; hit_j[k] = j0 + 8 * g + 4; hit_c[k] = c[2 * g + 1];
+                        }
+                        nhit += add;
                     }
-                    if (h1) {
-                        const int e = nhit + __popc(m0) + __popc(m1 & lt);
-                        hit_i[e] = pend.i; hit_j[e] = pend.j0 + 4; hit_c[e] = c.y;
-                    }
-                    nhit += add;
                 }
             } else {
-                // the warp holds 8 rows (r) x 8 columns (c4, c4 + 4): reduce over the columns for the row sums
-                // (kept in registers until the row changes) and over the rows for the column sums
-                float cx = pend.ok0 ? c.x : 0.0f, cy = pend.ok1 ? c.y : 0.0f;
-                int32_t bc = (pend.ok0 && c.x < P.sink.cutoff ? 1 : 0) | (pend.ok1 && c.y < P.sink.cutoff ? 1 << 16 : 0);
-                float rs = cx + cy;
-                int32_t rb = (bc & 0xffff) + (bc >> 16);
+                // the warp holds 8 rows (r) x 16 columns (c4 + 4 e): reduce over the columns for the row sums (kept in
+                // registers until the row changes) and over the rows for the column sums
+                float cv[4];
+                int32_t bc[2] = {0, 0};                          // below-counts of columns (0, 1) and (2, 3), 16 bits each
+                float rs = 0.0f;
+                int32_t rb = 0;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    cv[e] = ok[e] ? c[e] : 0.0f;
+                    const int32_t b = ok[e] && c[e] < P.sink.cutoff ? 1 : 0;
+                    rs += cv[e];
+                    rb += b;
+                    bc[e >> 1] |= b << (16 * (e & 1));
+                }
 #pragma unroll
                 for (int o = 1; o <= 2; o <<= 1) {
                     rs += __shfl_xor_sync(0xffffffffu, rs, o);
                     rb += __shfl_xor_sync(0xffffffffu, rb, o);
                 }
-                if (pend.i != acc_i) {
+                if (i_cur != acc_i) {
                     flush_row();
-                    acc_i = pend.i;
+                    acc_i = i_cur;
                     acc_sum = 0.0;
                     acc_cnt = 0;
                 }
@@ -508,121 +600,23 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
                 acc_cnt += rb;
 #pragma unroll
                 for (int o = 4; o <= 16; o <<= 1) {
-                    cx += __shfl_xor_sync(0xffffffffu, cx, o);
-                    cy += __shfl_xor_sync(0xffffffffu, cy, o);
-                    bc += __shfl_xor_sync(0xffffffffu, bc, o);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) cv[e] += __shfl_xor_sync(0xffffffffu, cv[e], o);
+                    bc[0] += __shfl_xor_sync(0xffffffffu, bc[0], o);
+                    bc[1] += __shfl_xor_sync(0xffffffffu, bc[1], o);
                 }
                 if (r == 0) {
-                    if (pend.j0 < (int32_t)P.N) {
-                        atomicAdd(P.sink.rowsum + pend.j0, (double)cx);
-                        if (bc & 0xffff) atomicAdd(P.sink.below + pend.j0, bc & 0xffff);
-                    }
-                    if (pend.j0 + 4 < (int32_t)P.N) {
-                        atomicAdd(P.sink.rowsum + pend.j0 + 4, (double)cy);
-                        if (bc >> 16) atomicAdd(P.sink.below + pend.j0 + 4, bc >> 16);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const int32_t j = j0 + 4 * e;
+                        const int32_t b = (bc[e >> 1] >> (16 * (e & 1))) & 0xffff;
+                        if (j < (int32_t)P.N) {
+                            atomicAdd(P.sink.rowsum + j, (double)cv[e]);
+                            if (b) atomicAdd(P.sink.below + j, b);
+                        }
                     }
                 }
             }
-        };
-        uint32_t buf = (uint32_t)team, acc_par = 0;             // this team's tile n: buffer n % NB, use number n / NB of it
-        auto tile_body = [&](Pending& pend, const Pending& prev, const bool have_prev) {
-            if (I != curI) {                                     // per-row quantities (warp-uniform branch)
-                curI = I;
-                i = I * I8_ROW_MODELS + quad * 8 + r;
-                row_ok = i < N32 && i >= (int32_t)P.row_begin && i < (int32_t)P.row_end;
-                const float* ri = P.cstat + (size_t)(i >> 4) * I8_CSTAT_TILE + i8_col_slot(i & 15);   // slots beyond N hold neutral records
-                // (the identity shuffles make the warp wait for these three loads HERE, in the rare row-change path: left
-                // pending, their scoreboard slot is shared with the per-tile loads below and the first read of si_* in
-                // every later tile then waits for those -- measured: 6 % of the epilogue's stall samples at L = 100)
-                si_Thi = __shfl_sync(0xffffffffu, ri[0], lane);
-                si_Tlo = __shfl_sync(0xffffffffu, ri[16], lane);
-                si_pw = __shfl_sync(0xffffffffu, ri[32], lane);
-                rowoff = (int64_t)i * (2 * P.N - i - 1) / 2 - i - 1 - P.base;
-            }
-            const int32_t j0 = J * I8_COL_MODELS + half * 8 + c4;
-            // records of this thread's two column models: three 8-byte loads that land directly in the register pairs
-            // the packed arithmetic reads (no moves, so nothing waits for them before the tile's finish, one tile later)
-            {
-                const float* cj = P.cstat + (size_t)J * I8_CSTAT_TILE + half * 8 + c4 * 2;
-                pend.Thj = *reinterpret_cast<const float2*>(cj);
-                pend.Tlj = *reinterpret_cast<const float2*>(cj + 16);
-                pend.pwj = *reinterpret_cast<const float2*>(cj + 32);
-            }
-            pend.Thi = si_Thi; pend.Tlo = si_Tlo; pend.pw = si_pw;
-            pend.dst = P.out + rowoff + j0;
-            pend.i = i;
-            pend.j0 = j0;
-            pend.ok0 = row_ok && j0 < N32 && j0 > i;             // masked pairs are simply not stored
-            pend.ok1 = row_ok && j0 + 4 < N32 && j0 + 4 > i;
-            // advance to the team's next tile (two tiles on)
-#pragma unroll
-            for (int s = 0; s < 2; ++s)
-                if (++J >= Tc32) { ++I; J = 2 * I; }
-            ptx::mbar_wait(ACC_FULL(buf), acc_par);
-            ptx::tc_fence_after();
-            const uint32_t ta = tmem + ((uint32_t)(quad * 32) << 16) + buf * I8_ACC_COLS + half * 8;
-            // m[3p+q] = (.x, .y): pairs (row model r, column model c4 + 8 half) and (.., + 4); Gram sums in units
-            // of 2^46.  The two pairs of a thread go through the closed form together, on packed fp32 arithmetic.
-            // The accumulator buffer is held only for the loads and the level recombination below and handed back
-            // to the MMA warp before any of the closed form runs (at L <= 128 the epilogue, not the tensor pipe, sets the
-            // pace: every cycle the buffer is held is a cycle the next tile's MMAs cannot start).
-            float2 m[9];
-            {
-                // levels 1 and 2 first: T = 2^8 V1 + V2 fits int32 (|T| < 2^31 for L <= 256 because |d0| <= 127)
-                uint32_t v1[3][2][4], v2[3][2][4], v0[3][2][4];
-#pragma unroll
-                for (int q = 0; q < 3; ++q)
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 48 + 16 * q, v1[q][h]);
-                        ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 96 + 16 * q, v2[q][h]);
-                    }
-                ptx::tmem_ld_wait();
-                // level 0 is requested before levels 1 and 2 are converted, so its latency is covered by that work
-#pragma unroll
-                for (int q = 0; q < 3; ++q)
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) ptx::tmem_ld_16x256b(ta + ((uint32_t)(16 * h) << 16) + 16 * q, v0[q][h]);
-                const float2 s30 = make_float2(0x1p-30f, 0x1p-30f);
-#pragma unroll
-                for (int q = 0; q < 3; ++q) {
-                    // register slots of a 16x256b load: [0,1] = lane r (h = 0: p = 0, h = 1: p = 2), [2,3] = lane r + 8 (p = 1)
-                    auto T = [&](int h, int e) { return (float)(((int32_t)v1[q][h][e] << 8) + (int32_t)v2[q][h][e]); };
-                    m[0 + q] = __fmul2_rn(make_float2(T(0, 0), T(0, 1)), s30);
-                    m[3 + q] = __fmul2_rn(make_float2(T(0, 2), T(0, 3)), s30);
-                    m[6 + q] = __fmul2_rn(make_float2(T(1, 0), T(1, 1)), s30);
-                }
-                ptx::tmem_ld_wait();
-                // the accumulator buffer is free again
-                ptx::tc_fence_before();
-                __syncwarp();
-                if (lane == 0) ptx::mbar_arrive(ACC_EMPTY(buf));
-                buf += 2;                                        // the team's next tile is two tiles on
-                if (buf >= (uint32_t)NB) { buf -= NB; acc_par ^= 1; }
-                const float2 s14 = make_float2(0x1p-14f, 0x1p-14f);
-#pragma unroll
-                for (int q = 0; q < 3; ++q) {
-                    auto F = [&](int h, int e) { return (float)(int32_t)v0[q][h][e]; };
-                    m[0 + q] = __ffma2_rn(make_float2(F(0, 0), F(0, 1)), s14, m[0 + q]);
-                    m[3 + q] = __ffma2_rn(make_float2(F(0, 2), F(0, 3)), s14, m[3 + q]);
-                    m[6 + q] = __ffma2_rn(make_float2(F(1, 0), F(1, 1)), s14, m[6 + q]);
-                }
-            }
-            // two independent chains: this tile's invariants and the previous tile's serial root-finding half
-            if (have_prev) finish_pending(prev);
-            pend.inv = eq2_invariants(m);
-        };
-        bool last_is_A = true;
-        for (uint32_t n = team; n < ntiles; n += 4) {
-            tile_body(pendA, pendB, have_pend);
-            have_pend = true;
-            last_is_A = true;
-            if (n + 2 >= ntiles) break;
-            tile_body(pendB, pendA, true);
-            last_is_A = false;
-        }
-        if (have_pend) {
-            if (last_is_A) finish_pending(pendA); else finish_pending(pendB);
         }
         if (MODE == SINK_ROWSTATS) flush_row();
         if (MODE == SINK_BELOW) flush_hits();
@@ -635,7 +629,7 @@ __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params
 static inline size_t i8tc_smem_bytes(int ks, int stages)
 {
     return (size_t)i8_a_stagings(ks) * 3 * ks * I8_A_SLAB + (size_t)stages * ks * I8_B_SLAB +
-           8 * (2 * stages + 4 + 2 * I8_MAX_ACC_BUFS) + 16;
+           8 * (2 * stages + 4 + I8_EPI_TEAMS + I8_MAX_ACC_BUFS) + 16;
 }
 static inline int i8tc_stages(int ks, size_t extra)
 {

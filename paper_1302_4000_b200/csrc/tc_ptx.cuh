@@ -160,6 +160,14 @@ __device__ __forceinline__ void tmem_ld_16x256b(uint32_t taddr, uint32_t v[4])
                  : "r"(taddr)
                  : "memory");
 }
+// the same twice along the columns: v[4..7] repeat v[0..3] eight columns further on
+__device__ __forceinline__ void tmem_ld_16x256b_x2(uint32_t taddr, uint32_t v[8])
+{
+    asm volatile("tcgen05.ld.sync.aligned.16x256b.x2.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+}
 // 32 lanes x 32 bit x 16 columns: thread t gets lane t, columns c..c+15
 __device__ __forceinline__ void tmem_ld_32x32b_x16(uint32_t taddr, uint32_t v[16])
 {
