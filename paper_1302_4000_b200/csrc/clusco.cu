@@ -90,10 +90,21 @@ int clusco_center(const float* coords, int64_t N, int32_t L, float* centred, flo
     if (!coords) return CLUSCO_ERR_INVALID_ARG;
     int st = check_device(nullptr);
     if (st != CLUSCO_OK) return st;
-    const int wpb = 8;
-    const int64_t blocks = (N + wpb - 1) / wpb;
-    if (blocks > 0x7fffffff) return CLUSCO_ERR_INVALID_ARG;
-    center_kernel<<<(unsigned)blocks, wpb * 32, 0, (cudaStream_t)stream>>>(coords, N, L, centred, r2);
+    // strip per warp: the model's 3 L floats plus the alignment lead, rounded to 16 bytes
+    const int64_t strip_floats = round_up(3 * (int64_t)L + 8, 4);
+    if (strip_floats <= CENTER_MAX_FLOATS) {
+        const int64_t blocks = (N + CENTER_WARPS - 1) / CENTER_WARPS;
+        if (blocks > 0x7fffffff) return CLUSCO_ERR_INVALID_ARG;
+        const size_t smem = (size_t)CENTER_WARPS * strip_floats * sizeof(float);
+        CLUSCO_CUDA_TRY(cudaFuncSetAttribute(center_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        center_kernel<<<(unsigned)blocks, CENTER_WARPS * 32, smem, (cudaStream_t)stream>>>(coords, N, L, (int32_t)strip_floats,
+                                                                                         centred, r2);
+    } else {
+        const int wpb = 8;
+        const int64_t blocks = (N + wpb - 1) / wpb;
+        if (blocks > 0x7fffffff) return CLUSCO_ERR_INVALID_ARG;
+        center_long_kernel<<<(unsigned)blocks, wpb * 32, 0, (cudaStream_t)stream>>>(coords, N, L, centred, r2);
+    }
     CLUSCO_CUDA_TRY(cudaGetLastError());
     return CLUSCO_OK;
 }

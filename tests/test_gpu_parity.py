@@ -64,6 +64,21 @@ def test_center_matches_oracle(clusco, c1):
     assert np.array_equal(x.cpu().numpy(), cen.cpu().numpy())
 
 
+@pytest.mark.parametrize("N,L", [(1, 1), (7, 2), (33, 5), (130, 77), (9, 887), (3, 4093), (5, 4500)])
+def test_center_ragged_shapes(clusco, N, L):
+    """Every alignment of a model's first float to the 16-byte vectors of the one-pass kernel (3 L n mod 4), chains up to
+    the strip capacity, and the two-pass kernel beyond it."""
+    rng = np.random.default_rng(1000 * N + L)
+    x = (rng.normal(size=(N, L, 3)) * 20 + rng.uniform(-50, 50, size=(N, 1, 3))).astype(np.float32)
+    cen, r2 = clusco.clusco_center(_dev(x))
+    cen_o, r2_o = oracle.center(x)
+    assert np.max(np.abs(cen.cpu().numpy().astype(np.float64) - cen_o)) <= 1.6e-5     # half an fp32 ulp at 128..256 A
+    if L > 1:
+        assert np.max(np.abs(r2.cpu().numpy() / r2_o - 1.0)) <= 2e-7
+    else:
+        assert np.all(r2.cpu().numpy() == 0.0)
+
+
 # ---- a3..a5 all-pairs: whole configs the oracle finishes in seconds ----------------------------------
 
 @pytest.mark.parametrize("cfg,N", [("C1", None), ("C2", None), ("C3", 1200), ("C4", 1500)])
