@@ -40,12 +40,9 @@ __host__ __device__ __forceinline__ int64_t packed_index(int64_t i, int64_t j, i
 // exact 2^k as float for k in [-126, 127]
 __device__ __forceinline__ float pow2i(int k) { return __int_as_float((k + 127) << 23); }
 
-// compact per-model record read by the epilogues with one 16-byte load
-struct __align__(16) PairStat {
-    float Thi, Tlo;     // two-float KAPPA^2 sum_k |a_k|^2 of the quantised coordinates, true scale (Angstrom^2)
-    float pw;           // 2^e, e = the model's scale exponent clamped to [-30, 30]
-    float pad;
-};
+// per-model epilogue records of the tensor-core engine (gram_i8tc.cuh: I8_CSTAT_TILE floats per column tile of 16 models,
+// [sum a^2 high | sum a^2 low | 2^e]); 16 bytes per model are reserved for them in the workspace
+constexpr int64_t I8_RECORD_BYTES_PER_MODEL = 16;
 
 // ---- what the fused all-pairs kernels do with a finished pair (i < j, c = cRMSD) ---------------------------
 // STORE:    out[packed index]                                   (a5, the matrix itself)
@@ -96,7 +93,7 @@ constexpr int I8_B_SLAB = 144 * 32;    // bytes of one k-step B slab: 3 digits x
 constexpr int I8_MAX_KSTEPS = 8;       // L <= 256: a row tile's A operand (3 digits x ksteps x 8 columns) stays resident in TMEM
 
 // ---- workspace layout --------------------------------------------------------------------------
-// [ ModelStat[Np] | PairStat[Np] | FFMA plane | i8 A planes | i8 B planes ]      Np = N rounded up to 128
+// [ ModelStat[Np] | i8 epilogue records | FFMA plane | i8 A planes | i8 B planes ]      Np = N rounded up to 128
 struct Workspace {
     int64_t N, Np;
     int32_t L;
@@ -120,7 +117,7 @@ static inline Workspace workspace_layout(int64_t N, int32_t L)
     w.off_stats = o;
     o += (size_t)round_up((int64_t)sizeof(ModelStat) * w.Np, 256);
     w.off_pstat = o;
-    o += (size_t)round_up((int64_t)sizeof(PairStat) * w.Np, 256);
+    o += (size_t)round_up(I8_RECORD_BYTES_PER_MODEL * w.Np, 256);
     w.off_ffma = o;                                        // float Yt[Lp16][3*Np]
     o += (size_t)round_up((int64_t)sizeof(float) * w.Lp16 * 3 * w.Np, 256);
     const int64_t ks = w.Lp32 / 32;
