@@ -109,3 +109,18 @@ def test_partition_rows(lib):
         if N >= 10000:
             pairs = [hi * (2 * N - hi - 1) // 2 - lo * (2 * N - lo - 1) // 2 for lo, hi in zip(b, b[1:])]
             assert max(pairs) < 1.15 * (N * (N - 1) // 2) / parts
+
+
+def test_i8tc_geometry_counts_the_upper_triangle_tiles():
+    """Row tile I (32 models) meets column tiles J >= 2 I (16 models each): the host-only geometry query must report exactly
+    that many tiles, the k-step count ceil(L / 32), and refuse chains the tensor-core engine does not serve."""
+    import paper_1302_4000_b200 as clusco
+    for N, L in ((2, 1), (33, 5), (200, 76), (2000, 120), (10000, 250), (30000, 100), (4097, 256)):
+        geo = clusco.i8tc_geometry(N, L)
+        rows, cols = (N + 31) // 32, (N + 15) // 16
+        assert geo["tiles"] == sum(max(0, cols - 2 * I) for I in range(rows))
+        assert geo["ksteps"] == (L + 31) // 32
+        assert geo["mma_columns_per_kstep"] == 144 + 96 + 48
+    assert clusco.engine_supported(clusco.ENGINE_I8TC, 256) and not clusco.engine_supported(clusco.ENGINE_I8TC, 257)
+    with pytest.raises(clusco.CluscoError):
+        clusco.i8tc_geometry(100, 300)
