@@ -43,7 +43,7 @@ template <int DIGITS> struct DGCfg {
     // padded to a multiple of it
     static constexpr int KG = DIGITS == 3 ? DG_KG3 : 4;
 };
-// CMO on the cluster path: every CTA owns a 2 x 2 block of 128-model tiles (profiles/r01g_next_rows.md has the history:
+// CMO on the cluster path: every CTA owns a 2 x 2 block of 128-model tiles (DESIGN.md section 13 has the history:
 // 3.1 ms -> 1.47 ms at C3's shape against 0.7 ms of tensor time)
 constexpr int DG_CMO_CLUSTER_I = 1;            // CMO cluster rows: 2 (2 x 2, 132 SMs) or 1 (1 x 2, all 148 SMs, 1.5 x the L2 reads)
 constexpr int DG_KG1B = 2;                     // CMO, blocked: k-steps per stage (measured: 2 -> 1.69 ms, 4 -> 1.71 ms whole call)
