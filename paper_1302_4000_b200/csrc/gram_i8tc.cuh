@@ -32,6 +32,7 @@
 #pragma once
 #include "common.cuh"
 #include "epilogue.cuh"
+#include "i8_layout.cuh"
 #include "prep.cuh"
 #include "tc_ptx.cuh"
 
@@ -77,7 +78,8 @@ static inline bool i8tc_supported(int32_t L) { return L >= 1 && L <= 32 * I8_MAX
 
 // ---- a1 + a2 + operand planes, one launch --------------------------------------------------------------------
 // Ap[row_tile][digit][kstep][I8_A_SLAB], Bp[col_tile][kstep][I8_B_SLAB]; a slab is a grid of 8-row x 16-byte core
-// matrices: byte (row, k) of a slab sits at (row/8)*256 + (k/16)*128 + (row%8)*16 + k%16.
+// matrices: byte (row, k) of a slab sits at (row/8)*256 + (k/16)*128 + (row%8)*16 + k%16  (i8_layout.cuh, whose functions
+// a host harness shares with this kernel: tests/test_i8_layout.py).
 // One warp per model slot.  The model is read ONCE, element-wise (coalesced), and stays in registers through
 // three passes: FP64 centroid -> max|a| (scale exponent) -> fixed-point integers I.  The integers of a round
 // (4 k-steps = 128 atoms) go through a warp-private shared-memory strip so that each lane can pack the digit
@@ -86,8 +88,6 @@ static inline bool i8tc_supported(int32_t L) { return L >= 1 && L <= 32 * I8_MAX
 // [Thi[16] | Tlo[16] | pw[16]] with model m of the tile at slot i8_col_slot(m) -- the order of the B rows -- so that the
 // two column models of an epilogue thread (c and c + 4) are adjacent: one 8-byte load per quantity.
 constexpr int I8_CSTAT_TILE = 48;
-__host__ __device__ __forceinline__ int i8_col_slot(int m16) { return (m16 & 8) | ((m16 & 3) << 1) | ((m16 >> 2) & 1); }
-__host__ __device__ __forceinline__ int i8_stat_slot(int m16) { return ((m16 & 3) << 2) | ((m16 >> 2) & 3); }
 constexpr int I8_PREP_WARPS = 8;
 constexpr int I8_PREP_STRIP = 4 * 97;          // ints per warp and round: 4 k-steps x (96 + 1 pad)
 
@@ -145,15 +145,11 @@ __global__ void __launch_bounds__(I8_PREP_WARPS * 32) i8_prep_kernel(const float
     ex = max(-30, min(30, ex));
     const double scale = valid ? ldexp(I8_KAPPA, 23 - ex) : 0.0;
 
-    // A image: row tile n/32, quadrant w = (n%32)/8, row-in-group r = n%8, row group 4w + p
-    const int64_t a_tile = n >> 5;
-    const int a_w = (int)(n & 31) >> 3, a_r = (int)(n & 7);
-    // B image: column tile n/16, o = position of this model among the 16 columns of a component block
+    // (A image: row tile n/32, quadrant w = (n%32)/8, row-in-group r = n%8, row group 4w + p; B image: column tile n/16,
+    // o = position of this model among the 16 columns of a component block -- i8_store_lane_words)
     const int64_t b_tile = n >> 4;
     const int m16 = (int)(n & 15);
-    const int b_o = i8_col_slot(m16);
     const int sub = lane >> 3, j = lane & 7;               // packing role: k-step 4 r + sub, atoms 4 j .. 4 j + 3 of it
-    const int kc = j >> 2, kb = (j & 3) * 4;
     int* strip = strip_s[wib];
     unsigned long long sumsq = 0ull;
 #pragma unroll
@@ -175,34 +171,15 @@ __global__ void __launch_bounds__(I8_PREP_WARPS * 32) i8_prep_kernel(const float
                 uint32_t w[3] = {0u, 0u, 0u};
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
-                    const int I = strip[97 * sub + 3 * (4 * j + i) + p];
-                    const int d2 = (int)(int8_t)(I & 0xff);
-                    const int I1 = (I - d2) >> 8;
-                    const int d1 = (int)(int8_t)(I1 & 0xff);
-                    const int d0 = (I1 - d1) >> 8;
+                    int d0, d1, d2;
+                    i8_digits(strip[97 * sub + 3 * (4 * j + i) + p], d0, d1, d2);
                     w[0] |= (uint32_t)(d0 & 0xff) << (8 * i);
                     w[1] |= (uint32_t)(d1 & 0xff) << (8 * i);
                     w[2] |= (uint32_t)(d2 & 0xff) << (8 * i);
                 }
-                if (n < row_slots) {
-#pragma unroll
-                    for (int a = 0; a < 3; ++a)
-                        *reinterpret_cast<uint32_t*>(Ap + ((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + p) * 256 +
-                                                     kc * 128 + a_r * 16 + kb) = w[a];
-                }
-                if (n < col_slots) {
-#pragma unroll
-                    for (int b = 0; b < 3; ++b)
-                        *reinterpret_cast<uint32_t*>(Bp + (b_tile * ks + kk) * I8_B_SLAB + b * 1536 +
-                                                     (2 * p + (b_o >> 3)) * 256 + kc * 128 + (b_o & 7) * 16 + kb) = w[b];
-                }
+                i8_store_lane_words(Ap, Bp, n < row_slots, n < col_slots, n, ks, kk, j, p, w[0], w[1], w[2]);
             }
-            if (n < row_slots) {                           // the zero rows (p = 3) of this model's quadrant
-#pragma unroll
-                for (int a = 0; a < 3; ++a)
-                    *reinterpret_cast<uint32_t*>(Ap + ((a_tile * 3 + a) * ks + kk) * I8_A_SLAB + (4 * a_w + 3) * 256 +
-                                                 kc * 128 + a_r * 16 + kb) = 0u;
-            }
+            i8_store_lane_words(Ap, Bp, n < row_slots, false, n, ks, kk, j, 3, 0u, 0u, 0u);      // the zero rows
         }
         __syncwarp();
     }
@@ -263,7 +240,6 @@ template <int KS, int MODE>
 __global__ void __launch_bounds__(I8_THREADS, 1) gram_i8tc_kernel(const I8Params P)
 {
     extern __shared__ __align__(128) uint8_t smem[];
-    constexpr int ks = KS;
     constexpr uint32_t STAGE_BYTES = KS * I8_B_SLAB;
     const int stages = P.stages;
     constexpr int NB = i8_acc_bufs(KS);
